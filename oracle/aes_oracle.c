@@ -139,10 +139,13 @@ void oracle_mix_columns(uint8_t state[16])
     for (c = 0; c < 4; c++) {
         uint8_t s0 = state[0 + 4 * c], s1 = state[1 + 4 * c];
         uint8_t s2 = state[2 + 4 * c], s3 = state[3 + 4 * c];
-        state[0 + 4 * c] = (uint8_t)(oracle_gf_mul(2, s0) ^ oracle_gf_mul(3, s1) ^ s2 ^ s3);
-        state[1 + 4 * c] = (uint8_t)(s0 ^ oracle_gf_mul(2, s1) ^ oracle_gf_mul(3, s2) ^ s3);
-        state[2 + 4 * c] = (uint8_t)(s0 ^ s1 ^ oracle_gf_mul(2, s2) ^ oracle_gf_mul(3, s3));
-        state[3 + 4 * c] = (uint8_t)(oracle_gf_mul(3, s0) ^ s1 ^ s2 ^ oracle_gf_mul(2, s3));
+        /* sec. 4.2.1: {02}*s = xtime(s); {03}*s = xtime(s) ^ s               */
+        uint8_t d0 = oracle_xtime(s0), d1 = oracle_xtime(s1);
+        uint8_t d2 = oracle_xtime(s2), d3 = oracle_xtime(s3);
+        state[0 + 4 * c] = (uint8_t)(d0 ^ (d1 ^ s1) ^ s2 ^ s3);
+        state[1 + 4 * c] = (uint8_t)(s0 ^ d1 ^ (d2 ^ s2) ^ s3);
+        state[2 + 4 * c] = (uint8_t)(s0 ^ s1 ^ d2 ^ (d3 ^ s3));
+        state[3 + 4 * c] = (uint8_t)((d0 ^ s0) ^ s1 ^ s2 ^ d3);
     }
 }
 
