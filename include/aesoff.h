@@ -1,0 +1,218 @@
+/*
+ * aesoff.h -- C ABI of the B200 AES-CTR offload engine.
+ *
+ * What this library is.  The paper's servers reroute one fine-grained routine to
+ * an accelerator: `accel_encrypt(j.buf, j.len)` (Listing 1), which
+ * "performs AES ... on its own CUDA stream, polled by cudaEventQuery, with the
+ * block size sweeping from 4 KiB (launch-bound) to 8 MiB (bandwidth-bound)"
+ * (section 6 "Experimental setup").  The calls below are that
+ * routine split along the paper's three-step recipe (section 3:
+ * "submit the work to a background executor instead of waiting", "suspend the
+ * current request", "resume it ... when the offload completes"):
+ *
+ *     submit  -> aes_ctr_submit()   returns a completion handle at once
+ *     suspend -> the caller's job (suspend BEFORE submitting)
+ *     resume  -> the caller's executor spins on aes_poll() / aes_wait()
+ *
+ * The paper fixes neither mode nor key size; BASELINE.json fixes AES-128 and
+ * AES-256 in CTR mode (SP 800-38A sec. 6.5 over FIPS-197), DESIGN.md lists every
+ * such reading.  No floating point anywhere: results are exact and unique.
+ *
+ * Conventions common to all calls
+ *   - Plain C types only.  "host" / "device" is stated for every pointer.
+ *   - One engine per process (one process per GPU).  All calls are thread-safe
+ *     unless stated; aes_ctr_submit() may be called from many executor threads
+ *     ("worker pool", "32-thread executor").
+ *   - Errors are negative ints (AES_E_*); a call that returns NULL / 0 leaves
+ *     the code in a thread-local slot read by aes_last_error().  Nothing aborts,
+ *     nothing throws.  There is NO CPU fallback: without a CUDA device every
+ *     compute call fails with AES_E_CUDA.
+ */
+#ifndef AESOFF_H
+#define AESOFF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+#if defined(__GNUC__)
+#pragma GCC visibility push(default)   /* the library itself is built with -fvisibility=hidden */
+#endif
+
+/* ---- error codes ---------------------------------------------------------- */
+#define AES_OK           0
+#define AES_E_INVAL     -1   /* NULL pointer, bad option value                      */
+#define AES_E_KEYBITS   -2   /* keybits not 128 or 256                             */
+#define AES_E_ALIGN     -3   /* src or dst not 16-byte aligned                     */
+#define AES_E_OVERLAP   -4   /* src/dst overlap partially (dst == src is allowed)  */
+#define AES_E_AGAIN     -5   /* submission ring full: retry after some completions */
+#define AES_E_TIMEOUT   -6   /* aes_wait() timed out                               */
+#define AES_E_STOPPED   -7   /* engine not running (never started, stopped, dead)  */
+#define AES_E_CUDA      -8   /* a CUDA runtime call failed / no device             */
+#define AES_E_BUSY      -9   /* call not allowed while the engine is running       */
+#define AES_E_NOMEM     -10  /* host or device allocation failed                   */
+
+typedef struct aes_ctx aes_ctx_t;     /* opaque; owns a copy of the expanded round keys */
+typedef uint64_t       aes_handle_t;  /* submission sequence number, from 1; 0 = invalid */
+
+/* ---- engine life cycle (step a0 of the path) -------------------------------
+ * The engine is: a pinned, host-mapped descriptor ring; ONE persistent sm_100a
+ * kernel (a dispatcher warp that polls the ring over PCIe plus worker groups
+ * that hold the AES tables in shared memory); and a host-mapped completion
+ * mailbox.  A request therefore never pays a kernel launch (the paper's 4 KiB
+ * point is "launch-bound").                                       */
+typedef struct aes_engine_opts {
+    uint32_t ring_slots;      /* descriptor ring depth = max requests in flight; power of
+                                 two in [64, 4096]; 0 = default 2048                      */
+    uint32_t chunk_rows;      /* work-item size in 4 KiB rows (256 counter values each);
+                                 1..64; 0 = default 4 (16 KiB per worker-group item)      */
+    uint32_t n_ctas;          /* persistent CTAs; 0 = one per SM                          */
+    uint32_t idle_exit_ms;    /* the kernel exits by itself (engine becomes STOPPED) after
+                                 this long with no request; 0 = never                     */
+    uint32_t reserved[4];     /* must be 0                                                */
+} aes_engine_opts_t;
+
+/* Starts the engine on CUDA device `device`.  opts == NULL means all defaults.
+ * Returns AES_OK, AES_E_BUSY if already running, AES_E_INVAL, AES_E_CUDA, AES_E_NOMEM.
+ * While the engine runs, a device-wide synchronisation (cudaDeviceSynchronize,
+ * cudaFree, torch.cuda.synchronize) blocks until aes_engine_stop(): synchronise
+ * on streams or events instead.                                                  */
+int aes_engine_start(int device, const aes_engine_opts_t *opts);
+
+/* Waits for every accepted request to complete, makes the persistent kernel exit,
+ * frees ring and mailbox.  Handles issued before the stop keep answering
+ * aes_poll() == 1.  Returns AES_OK or AES_E_STOPPED / AES_E_CUDA.                 */
+int aes_engine_stop(void);
+
+typedef struct aes_engine_info {
+    int32_t  running;            /* 1 while the persistent kernel is alive           */
+    int32_t  device;
+    int32_t  sm_count;
+    int32_t  n_ctas;
+    int32_t  threads_per_cta;
+    int32_t  groups_per_cta;     /* worker groups (128 threads each) per CTA         */
+    uint32_t ring_slots;
+    uint32_t chunk_rows;
+    uint32_t smem_bytes_per_cta;
+    uint32_t reserved0;
+    uint64_t submitted;          /* requests accepted so far                         */
+    uint64_t completed;          /* requests whose completion the host has observed
+                                    through aes_poll/aes_wait, lower bound            */
+    uint64_t kernel_launches;    /* CUDA kernels this library launched so far         */
+} aes_engine_info_t;
+int aes_engine_info(aes_engine_info_t *out);     /* host pointer; AES_OK / AES_E_INVAL */
+
+/* ---- key expansion (step a1; FIPS-197 sec. 5.2) -----------------------------
+ * key: host pointer to keybits/8 bytes, copied.  keybits in {128, 256}.
+ * Returns NULL on error (AES_E_INVAL, AES_E_KEYBITS, AES_E_NOMEM).  Needs no GPU and
+ * no running engine; cheap enough to sit on the request path (BASELINE.json
+ * configs[3] creates one ctx per request).  The expanded key travels inside each
+ * descriptor, so a ctx may be destroyed as soon as its last submit has returned. */
+aes_ctx_t *aes_ctx_create(const uint8_t *key, int keybits);
+void       aes_ctx_destroy(aes_ctx_t *ctx);      /* NULL is a no-op */
+
+/* Copies the 16*(Nr+1) round-key bytes (FIPS-197 byte order: round key r is
+ * bytes 16r..16r+15) to `out` (host, >= 240 bytes) and returns Nr (10 or 14), or
+ * AES_E_INVAL.  Exists so that tests can pin the key schedule on its own.         */
+int aes_ctx_round_keys(const aes_ctx_t *ctx, uint8_t *out);
+
+/* ---- submit (steps a2..a6; SP 800-38A sec. 6.5) -----------------------------
+ * Encrypts (= decrypts) len bytes: dst[i] = src[i] xor O[i], where O is the
+ * concatenation of Cipher_K(T_1), Cipher_K(T_2), ... with T_1 = nonce and
+ * T_{j+1} = (T_j + 1) mod 2^128 read as a big-endian integer; a final partial
+ * block uses the leading len mod 16 bytes of its O_n.  No padding.
+ *
+ *   ctx    host; round keys are copied into the descriptor before this returns.
+ *   nonce  host; the FULL 16-byte initial counter block T_1 (BASELINE.json
+ *          configs[0]: 8-byte nonce || 8-byte big-endian counter from 0); copied.
+ *   src    DEVICE pointer on the engine's GPU, or pinned host memory that the GPU
+ *          can address (cudaHostAlloc / aes_host_alloc: the kernel then reads it
+ *          over PCIe).  16-byte aligned.  Must stay valid and unchanged until
+ *          completion.
+ *   dst    same kinds of memory, 16-byte aligned, len bytes.  dst == src (in
+ *          place) is allowed; any other overlap is AES_E_OVERLAP.
+ *   len    any value >= 0; len == 0 completes without touching memory.
+ *
+ * Never blocks.  Returns the handle (>= 1), or 0 with aes_last_error() in
+ * {AES_E_INVAL, AES_E_ALIGN, AES_E_OVERLAP, AES_E_AGAIN (ring full), AES_E_STOPPED}.
+ * Requests may complete out of order.                                            */
+aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16],
+                            const void *src, void *dst, size_t len);
+
+/* ---- completion (step a7) ----------------------------------------------------
+ * aes_poll: 1 = complete, 0 = pending, < 0 = error (AES_E_INVAL for a handle that
+ * was never issued, AES_E_STOPPED if the engine died with the request pending).
+ * Wait-free: one acquire load of the host-mapped mailbox.  Once it has returned 1,
+ * every byte of dst is visible to any copy or kernel issued afterwards on any
+ * stream of the device, and to the host if dst is host memory.
+ * aes_wait: spins on aes_poll for at most timeout_ns (UINT64_MAX = forever).
+ * Returns AES_OK, AES_E_TIMEOUT or the aes_poll error.                             */
+int aes_poll(aes_handle_t h);
+int aes_wait(aes_handle_t h, uint64_t timeout_ns);
+
+int         aes_last_error(void);          /* thread-local; AES_OK if none          */
+const char *aes_strerror(int code);        /* static string                         */
+
+/* ---- launch backend: the paper's own mechanism, for comparison and profiling --
+ * "on its own CUDA stream, polled by cudaEventQuery".  Enqueues, on
+ * `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ * stream), one host->device copy of n descriptors followed by ONE ordinary launch
+ * of the same worker code the persistent engine runs, which processes the n
+ * requests and exits.  Returns after enqueueing; the caller synchronises the
+ * stream or an event.  Arrays are host pointers of n entries (nonces: 16*n
+ * bytes); src/dst entries as for aes_ctr_submit.  ctxs[i] may repeat.  The
+ * persistent engine must NOT be running (its CTAs hold the shared memory):
+ * AES_E_BUSY.  chunk_rows as in aes_engine_opts_t (0 = default).  An ordinary
+ * launch is what `ncu` can replay, so the committed profiles use this call.       */
+int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonces,
+                         const void *const *srcs, void *const *dsts,
+                         const size_t *lens, size_t n,
+                         int device, void *cuda_stream, uint32_t chunk_rows);
+
+/* ---- pinned host memory the GPU can address (for host-resident payloads) ----- */
+void *aes_host_alloc(size_t bytes);        /* NULL on error (AES_E_CUDA / AES_E_NOMEM) */
+void  aes_host_free(void *p);
+
+/* ---- closed-loop executor (the paper's worker pool) ----
+ * Drives the running engine from native code so that a microsecond offload is not
+ * measured through an interpreter: keeps `window` requests in flight ("submit the
+ * next on each completion"), one submitter thread that also polls, and records
+ * per-request submit->completion-observed latency.  With keys != NULL a fresh ctx
+ * is created (key expansion) and destroyed per request INSIDE the timed loop
+ * (BASELINE.json configs[3]); otherwise ctx is shared.  All arrays are host
+ * pointers with n entries (nonces: 16*n bytes; keys: 32*n bytes, 16 used when
+ * keybits[i] == 128).  lat_ns may be NULL.  `repeat` runs the n requests that many
+ * times back to back in one timed region (>= 1).                                   */
+typedef struct aes_loop_spec {
+    size_t              n;
+    uint32_t            window;
+    uint32_t            repeat;
+    aes_ctx_t          *ctx;        /* shared ctx, used when keys == NULL            */
+    const uint8_t      *keys;       /* optional per-request raw keys, 32-byte stride */
+    const int32_t      *keybits;    /* with keys: 128 or 256 per request             */
+    const uint8_t      *nonces;
+    const void *const  *srcs;
+    void *const        *dsts;
+    const size_t       *lens;
+} aes_loop_spec_t;
+
+typedef struct aes_loop_result {
+    uint64_t elapsed_ns;       /* first submit -> last completion observed           */
+    uint64_t bytes;            /* payload bytes completed                             */
+    uint64_t requests;         /* requests completed (n * repeat)                     */
+    uint64_t ring_full_spins;  /* times submit returned AES_E_AGAIN                   */
+    uint64_t max_in_flight;
+} aes_loop_result_t;
+
+/* Returns AES_OK or the first error.  lat_ns: host, n*repeat doubles or NULL.      */
+int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res, double *lat_ns);
+
+#if defined(__GNUC__)
+#pragma GCC visibility pop
+#endif
+#ifdef __cplusplus
+}
+#endif
+#endif /* AESOFF_H */

@@ -1,0 +1,235 @@
+"""Thin ctypes binding of include/aesoff.h -- argument marshalling only.
+
+Every step of the path (key expansion, submission ring, dispatch, counter blocks,
+cipher, XOR/store, completion) runs inside ``libaesoff.so``; nothing here
+computes.  The function names are those of the C ABI.  There is no CPU fallback:
+if the shared library is missing this module raises at import, and on a machine
+without a CUDA device every compute call fails with ``AES_E_CUDA``.
+
+Pointers are plain integers (``tensor.data_ptr()`` for device memory, the address
+returned by ``aes_host_alloc`` for pinned host memory).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libaesoff.so")
+
+AES_OK = 0
+AES_E_INVAL = -1
+AES_E_KEYBITS = -2
+AES_E_ALIGN = -3
+AES_E_OVERLAP = -4
+AES_E_AGAIN = -5
+AES_E_TIMEOUT = -6
+AES_E_STOPPED = -7
+AES_E_CUDA = -8
+AES_E_BUSY = -9
+AES_E_NOMEM = -10
+
+
+class AesOffError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__("%s: %s (%d)" % (where, aes_strerror(code), code))
+
+
+class aes_engine_opts_t(ctypes.Structure):
+    _fields_ = [("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32), ("n_ctas", ctypes.c_uint32),
+                ("idle_exit_ms", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 4)]
+
+
+class aes_engine_info_t(ctypes.Structure):
+    _fields_ = [("running", ctypes.c_int32), ("device", ctypes.c_int32), ("sm_count", ctypes.c_int32),
+                ("n_ctas", ctypes.c_int32), ("threads_per_cta", ctypes.c_int32), ("groups_per_cta", ctypes.c_int32),
+                ("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32),
+                ("smem_bytes_per_cta", ctypes.c_uint32), ("reserved0", ctypes.c_uint32),
+                ("submitted", ctypes.c_uint64), ("completed", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64)]
+
+
+class aes_loop_spec_t(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_size_t), ("window", ctypes.c_uint32), ("repeat", ctypes.c_uint32),
+                ("ctx", ctypes.c_void_p), ("keys", ctypes.c_void_p), ("keybits", ctypes.c_void_p),
+                ("nonces", ctypes.c_void_p), ("srcs", ctypes.c_void_p), ("dsts", ctypes.c_void_p),
+                ("lens", ctypes.c_void_p)]
+
+
+class aes_loop_result_t(ctypes.Structure):
+    _fields_ = [("elapsed_ns", ctypes.c_uint64), ("bytes", ctypes.c_uint64), ("requests", ctypes.c_uint64),
+                ("ring_full_spins", ctypes.c_uint64), ("max_in_flight", ctypes.c_uint64)]
+
+
+def _load() -> ctypes.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "%s is missing: build it with `python -m paper_2607_02630_b200.build` "
+            "(or __graft_entry__.build()).  There is no CPU fallback." % LIB_PATH)
+    L = ctypes.CDLL(LIB_PATH)
+    vp, u64, i32, sz = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int, ctypes.c_size_t
+    sigs = {
+        "aes_engine_start": (i32, [i32, vp]),
+        "aes_engine_stop": (i32, []),
+        "aes_engine_info": (i32, [vp]),
+        "aes_ctx_create": (vp, [vp, i32]),
+        "aes_ctx_destroy": (None, [vp]),
+        "aes_ctx_round_keys": (i32, [vp, vp]),
+        "aes_ctr_submit": (u64, [vp, vp, vp, vp, sz]),
+        "aes_poll": (i32, [u64]),
+        "aes_wait": (i32, [u64, u64]),
+        "aes_last_error": (i32, []),
+        "aes_strerror": (ctypes.c_char_p, [i32]),
+        "aes_ctr_launch_batch": (i32, [vp, vp, vp, vp, vp, sz, i32, vp, ctypes.c_uint32]),
+        "aes_host_alloc": (vp, [sz]),
+        "aes_host_free": (None, [vp]),
+        "aes_loop_run": (i32, [vp, vp, vp]),
+    }
+    for name, (res, args) in sigs.items():
+        fn = getattr(L, name)
+        fn.restype = res
+        fn.argtypes = args
+    return L
+
+
+_lib = _load()
+EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_ctx_create", "aes_ctx_destroy",
+           "aes_ctx_round_keys", "aes_ctr_submit", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
+           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run")
+
+
+def aes_strerror(code: int) -> str:
+    return _lib.aes_strerror(code).decode()
+
+
+def aes_last_error() -> int:
+    return _lib.aes_last_error()
+
+
+def _check(rc: int, where: str) -> None:
+    if rc != AES_OK:
+        raise AesOffError(rc, where)
+
+
+# ---- engine ---------------------------------------------------------------------------------
+def aes_engine_start(device: int = 0, ring_slots: int = 0, chunk_rows: int = 0, n_ctas: int = 0,
+                     idle_exit_ms: int = 0) -> None:
+    o = aes_engine_opts_t(ring_slots, chunk_rows, n_ctas, idle_exit_ms)
+    _check(_lib.aes_engine_start(device, ctypes.byref(o)), "aes_engine_start")
+
+
+def aes_engine_stop() -> None:
+    _check(_lib.aes_engine_stop(), "aes_engine_stop")
+
+
+def aes_engine_info() -> dict:
+    info = aes_engine_info_t()
+    _check(_lib.aes_engine_info(ctypes.byref(info)), "aes_engine_info")
+    return {k: getattr(info, k) for k, _ in aes_engine_info_t._fields_ if k != "reserved0"}
+
+
+# ---- contexts ---------------------------------------------------------------------------------
+def aes_ctx_create(key: bytes, keybits: int | None = None) -> int:
+    key = bytes(key)
+    ctx = _lib.aes_ctx_create(key, 8 * len(key) if keybits is None else keybits)
+    if not ctx:
+        raise AesOffError(aes_last_error(), "aes_ctx_create")
+    return ctx
+
+
+def aes_ctx_destroy(ctx: int) -> None:
+    _lib.aes_ctx_destroy(ctx)
+
+
+def aes_ctx_round_keys(ctx: int) -> tuple:
+    buf = ctypes.create_string_buffer(240)
+    nr = _lib.aes_ctx_round_keys(ctx, buf)
+    if nr < 0:
+        raise AesOffError(nr, "aes_ctx_round_keys")
+    return buf.raw[: 16 * (nr + 1)], nr
+
+
+# ---- submit / completion ------------------------------------------------------------------------
+def aes_ctr_submit(ctx: int, nonce: bytes, src: int, dst: int, length: int) -> int:
+    """Returns the handle; raises AesOffError (code AES_E_AGAIN when the ring is full)."""
+    h = _lib.aes_ctr_submit(ctx, bytes(nonce), src, dst, length)
+    if h == 0:
+        raise AesOffError(aes_last_error(), "aes_ctr_submit")
+    return h
+
+
+def aes_poll(handle: int) -> bool:
+    r = _lib.aes_poll(handle)
+    if r < 0:
+        raise AesOffError(r, "aes_poll")
+    return r == 1
+
+
+def aes_wait(handle: int, timeout_ns: int = 10_000_000_000) -> None:
+    _check(_lib.aes_wait(handle, timeout_ns), "aes_wait")
+
+
+# ---- launch backend -----------------------------------------------------------------------------
+def _ptr_array(values) -> np.ndarray:
+    return np.ascontiguousarray(np.asarray(values, dtype=np.uint64))
+
+
+def aes_ctr_launch_batch(ctxs, nonces, srcs, dsts, lens, device: int = 0, cuda_stream: int = 0,
+                         chunk_rows: int = 0) -> None:
+    """ctxs/srcs/dsts/lens: sequences of n ints; nonces: n x 16 bytes (bytes or uint8 array)."""
+    n = len(lens)
+    a_ctx, a_src, a_dst, a_len = _ptr_array(ctxs), _ptr_array(srcs), _ptr_array(dsts), _ptr_array(lens)
+    a_non = np.ascontiguousarray(np.frombuffer(bytes(nonces), dtype=np.uint8) if isinstance(nonces, (bytes, bytearray))
+                                 else np.asarray(nonces, dtype=np.uint8)).reshape(-1)
+    assert a_non.size == 16 * n and a_ctx.size == n and a_src.size == n and a_dst.size == n
+    _check(_lib.aes_ctr_launch_batch(a_ctx.ctypes.data, a_non.ctypes.data, a_src.ctypes.data, a_dst.ctypes.data,
+                                     a_len.ctypes.data, n, device, cuda_stream, chunk_rows), "aes_ctr_launch_batch")
+
+
+# ---- pinned host memory ---------------------------------------------------------------------------
+def aes_host_alloc(nbytes: int) -> int:
+    p = _lib.aes_host_alloc(nbytes)
+    if not p:
+        raise AesOffError(aes_last_error(), "aes_host_alloc")
+    return p
+
+
+def aes_host_free(ptr: int) -> None:
+    _lib.aes_host_free(ptr)
+
+
+def host_view(ptr: int, nbytes: int) -> np.ndarray:
+    """uint8 numpy view of memory returned by aes_host_alloc (no copy)."""
+    return np.ctypeslib.as_array((ctypes.c_uint8 * nbytes).from_address(ptr))
+
+
+# ---- closed-loop executor ---------------------------------------------------------------------------
+def aes_loop_run(nonces, srcs, dsts, lens, window: int, ctx: int = 0, keys=None, keybits=None, repeat: int = 1,
+                 want_latency: bool = True) -> dict:
+    """Runs the native closed loop (see aes_loop_run in aesoff.h).  keys: n x 32 uint8 (16 used for
+    128-bit keys) with keybits: n int32, or a shared ``ctx``.  Returns elapsed_ns, bytes, requests,
+    ring_full_spins, max_in_flight and (optionally) lat_ns as a float64 array of n*repeat entries."""
+    n = len(lens)
+    a_src, a_dst, a_len = _ptr_array(srcs), _ptr_array(dsts), _ptr_array(lens)
+    a_non = np.ascontiguousarray(np.asarray(nonces, dtype=np.uint8)).reshape(-1)
+    assert a_non.size == 16 * n
+    spec = aes_loop_spec_t()
+    spec.n, spec.window, spec.repeat = n, window, repeat
+    spec.ctx = ctx or None
+    keep = []
+    if keys is not None:
+        a_keys = np.ascontiguousarray(np.asarray(keys, dtype=np.uint8)).reshape(-1)
+        a_kb = np.ascontiguousarray(np.asarray(keybits, dtype=np.int32))
+        assert a_keys.size == 32 * n and a_kb.size == n
+        spec.keys, spec.keybits = a_keys.ctypes.data, a_kb.ctypes.data
+        keep += [a_keys, a_kb]
+    spec.nonces, spec.srcs, spec.dsts, spec.lens = a_non.ctypes.data, a_src.ctypes.data, a_dst.ctypes.data, a_len.ctypes.data
+    res = aes_loop_result_t()
+    lat = np.zeros(n * repeat, dtype=np.float64) if want_latency else None
+    _check(_lib.aes_loop_run(ctypes.byref(spec), ctypes.byref(res), lat.ctypes.data if lat is not None else None),
+           "aes_loop_run")
+    out = {k: getattr(res, k) for k, _ in aes_loop_result_t._fields_}
+    out["lat_ns"] = lat
+    return out

@@ -1,0 +1,658 @@
+/*
+ * aesoff_runtime.cpp -- host runtime behind include/aesoff.h: engine life cycle, the multi-producer
+ * submission ring (step a2), the completion mailbox (step a7), the launch backend and the
+ * closed-loop executor.  Follows the paper's statement of the problem:
+ * submit returns at once, the caller suspends, an executor polls and resumes.
+ *
+ * Memory-model contract with the kernel (aesoff_kernels.cu):
+ *   host: write slot body; release-store slot.seq          GPU: ld.acquire.sys seq; read body
+ *   GPU : dst stores; bar; leader fence.sys; store mailbox  host: acquire-load mailbox[slot] >= seq
+ * A slot is reused for seq + R only after mailbox[slot] >= seq has been observed by the submitter.
+ */
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#include <time.h>
+
+#include <atomic>
+#include <mutex>
+#include <vector>
+
+#if defined(__x86_64__)
+#include <immintrin.h>
+#define CPU_RELAX() _mm_pause()
+#else
+#define CPU_RELAX() ((void)0)
+#endif
+
+#include "../../include/aesoff.h"
+#include "aesoff_internal.h"
+
+namespace {
+
+thread_local int t_last_error = AES_OK;
+inline int fail(int code)
+{
+    t_last_error = code;
+    return code;
+}
+
+inline uint64_t now_ns()
+{
+    struct timespec ts;
+    clock_gettime(CLOCK_MONOTONIC_RAW, &ts);
+    return (uint64_t)ts.tv_sec * 1000000000ull + (uint64_t)ts.tv_nsec;
+}
+
+struct Engine {
+    std::atomic<int> running{0};
+    int device = -1;
+    int sm_count = 0;
+    int n_ctas = 0;
+    uint32_t R = 0, Rm = 0, chunk_rows = 0, TM = 0;
+    cudaStream_t stream = nullptr;
+    aesoff_host_slot_t *hring = nullptr; /* pinned, mapped */
+    uint64_t *hmail = nullptr;           /* pinned, mapped */
+    uint32_t *hctl = nullptr;            /* pinned, mapped */
+    aesoff_dev_desc_t *dq = nullptr;
+    uint64_t *tmap = nullptr, *counters = nullptr, *dev_done_seq = nullptr;
+    uint32_t *dq_done = nullptr, *dT0 = nullptr;
+    uint64_t first_seq = 1;               /* first sequence number of the current run          */
+    std::atomic<uint64_t> next_seq{1};    /* next sequence number to hand out (never reset)    */
+};
+
+Engine g_eng;
+std::mutex g_lifecycle;
+std::atomic<uint64_t> g_kernel_launches{0};
+
+inline bool engine_dead(const Engine &e)
+{
+    return __atomic_load_n(&e.hctl[AESOFF_CTL_ALIVE], __ATOMIC_ACQUIRE) == 2u;
+}
+
+void free_engine_memory(Engine &e)
+{
+    if (e.hring) cudaFreeHost(e.hring);
+    if (e.hmail) cudaFreeHost(e.hmail);
+    if (e.hctl) cudaFreeHost(e.hctl);
+    if (e.dq) cudaFree(e.dq);
+    if (e.tmap) cudaFree(e.tmap);
+    if (e.counters) cudaFree(e.counters);
+    if (e.dev_done_seq) cudaFree(e.dev_done_seq);
+    if (e.dq_done) cudaFree(e.dq_done);
+    if (e.dT0) cudaFree(e.dT0);
+    if (e.stream) cudaStreamDestroy(e.stream);
+    e.hring = nullptr;
+    e.hmail = nullptr;
+    e.hctl = nullptr;
+    e.dq = nullptr;
+    e.tmap = e.counters = e.dev_done_seq = nullptr;
+    e.dq_done = e.dT0 = nullptr;
+    e.stream = nullptr;
+}
+
+inline bool is_pow2(uint32_t x) { return x && !(x & (x - 1)); }
+
+/* geometry of a request, the same arithmetic the dispatcher warp does on the device */
+inline void request_geometry(uint64_t len, uint8_t c0, uint32_t chunk_rows, uint32_t TM, uint64_t *rows,
+                             uint32_t *crows, uint32_t *nchunks)
+{
+    const uint64_t nblocks = (len >> 4) + ((len & 15) ? 1 : 0);
+    const uint64_t r = nblocks ? ((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0;
+    uint32_t cr = chunk_rows;
+    const uint64_t max_chunks = TM / 4;
+    while (((r + cr - 1) / cr) > max_chunks) cr *= 2;
+    *rows = r;
+    *crows = cr;
+    *nchunks = (uint32_t)((r + cr - 1) / cr);
+}
+
+int check_buffers(const void *src, void *dst, size_t len)
+{
+    if (len == 0) return AES_OK;
+    if (!src || !dst) return AES_E_INVAL;
+    const uintptr_t s = (uintptr_t)src, d = (uintptr_t)dst;
+    if ((s | d) & 15u) return AES_E_ALIGN;
+    if (s != d && s < d + len && d < s + len) return AES_E_OVERLAP;
+    return AES_OK;
+}
+
+} /* namespace */
+
+/* ============================================================================================ */
+/* errors                                                                                       */
+/* ============================================================================================ */
+extern "C" int aes_last_error(void) { return t_last_error; }
+
+extern "C" const char *aes_strerror(int code)
+{
+    switch (code) {
+    case AES_OK: return "ok";
+    case AES_E_INVAL: return "invalid argument";
+    case AES_E_KEYBITS: return "keybits must be 128 or 256";
+    case AES_E_ALIGN: return "src/dst must be 16-byte aligned";
+    case AES_E_OVERLAP: return "src and dst overlap partially";
+    case AES_E_AGAIN: return "submission ring full";
+    case AES_E_TIMEOUT: return "timed out";
+    case AES_E_STOPPED: return "engine not running";
+    case AES_E_CUDA: return "CUDA error or no device";
+    case AES_E_BUSY: return "not allowed while the engine is running";
+    case AES_E_NOMEM: return "out of memory";
+    default: return "unknown error";
+    }
+}
+
+/* ============================================================================================ */
+/* contexts (step a1)                                                                           */
+/* ============================================================================================ */
+extern "C" aes_ctx_t *aes_ctx_create(const uint8_t *key, int keybits)
+{
+    if (!key) {
+        fail(AES_E_INVAL);
+        return nullptr;
+    }
+    if (keybits != 128 && keybits != 256) {
+        fail(AES_E_KEYBITS);
+        return nullptr;
+    }
+    aes_ctx_t *c = (aes_ctx_t *)malloc(sizeof(aes_ctx_t));
+    if (!c) {
+        fail(AES_E_NOMEM);
+        return nullptr;
+    }
+    c->nr = aesoff_key_expand(key, keybits, c->rk);
+    c->keybits = keybits;
+    return c;
+}
+
+extern "C" void aes_ctx_destroy(aes_ctx_t *ctx) { free(ctx); }
+
+extern "C" int aes_ctx_round_keys(const aes_ctx_t *ctx, uint8_t *out)
+{
+    if (!ctx || !out) return fail(AES_E_INVAL);
+    /* little-endian words back to the FIPS-197 byte string */
+    for (int i = 0; i < 4 * (ctx->nr + 1); ++i) {
+        out[4 * i + 0] = (uint8_t)(ctx->rk[i]);
+        out[4 * i + 1] = (uint8_t)(ctx->rk[i] >> 8);
+        out[4 * i + 2] = (uint8_t)(ctx->rk[i] >> 16);
+        out[4 * i + 3] = (uint8_t)(ctx->rk[i] >> 24);
+    }
+    return ctx->nr;
+}
+
+/* ============================================================================================ */
+/* engine life cycle (step a0)                                                                  */
+/* ============================================================================================ */
+extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
+{
+    std::lock_guard<std::mutex> lk(g_lifecycle);
+    Engine &e = g_eng;
+    if (e.running.load()) return fail(AES_E_BUSY);
+
+    aes_engine_opts_t o;
+    memset(&o, 0, sizeof(o));
+    if (opts) o = *opts;
+    for (int i = 0; i < 4; ++i)
+        if (o.reserved[i]) return fail(AES_E_INVAL);
+    if (o.ring_slots == 0) o.ring_slots = 2048;
+    if (o.chunk_rows == 0) o.chunk_rows = 4;
+    if (!is_pow2(o.ring_slots) || o.ring_slots < 64 || o.ring_slots > 4096) return fail(AES_E_INVAL);
+    if (o.chunk_rows > 64) return fail(AES_E_INVAL);
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(AES_E_CUDA);
+    if (cudaSetDevice(device) != cudaSuccess) return fail(AES_E_CUDA);
+    int sms = 0, major = 0;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
+    if (major != 10) return fail(AES_E_CUDA); /* sm_100a code only */
+
+    e.device = device;
+    e.sm_count = sms;
+    e.n_ctas = o.n_ctas ? (int)o.n_ctas : sms;
+    e.R = o.ring_slots;
+    e.Rm = e.R - 1;
+    e.chunk_rows = o.chunk_rows;
+    e.TM = 1u << 18;
+    e.first_seq = e.next_seq.load();
+
+    bool ok = true;
+    ok = ok && cudaStreamCreateWithFlags(&e.stream, cudaStreamNonBlocking) == cudaSuccess;
+    const unsigned hflags = cudaHostAllocMapped | cudaHostAllocPortable;
+    ok = ok && cudaHostAlloc((void **)&e.hring, (size_t)e.R * sizeof(aesoff_host_slot_t), hflags) == cudaSuccess;
+    ok = ok && cudaHostAlloc((void **)&e.hmail, (size_t)e.R * 8, hflags) == cudaSuccess;
+    ok = ok && cudaHostAlloc((void **)&e.hctl, AESOFF_CTL_WORDS * 4, hflags) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.dq, (size_t)e.R * sizeof(aesoff_dev_desc_t)) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.tmap, (size_t)e.TM * 8) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.counters, AESOFF_CNT_WORDS * 8) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.dev_done_seq, (size_t)e.R * 8) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.dq_done, (size_t)e.R * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.dT0, 256 * 4) == cudaSuccess;
+    if (!ok) {
+        free_engine_memory(e);
+        return fail(AES_E_NOMEM);
+    }
+    memset(e.hring, 0, (size_t)e.R * sizeof(aesoff_host_slot_t));
+    memset(e.hmail, 0, (size_t)e.R * 8);
+    memset(e.hctl, 0, AESOFF_CTL_WORDS * 4);
+    ok = ok && cudaMemset(e.counters, 0, AESOFF_CNT_WORDS * 8) == cudaSuccess;
+    ok = ok && cudaMemset(e.dev_done_seq, 0, (size_t)e.R * 8) == cudaSuccess;
+    ok = ok && cudaMemset(e.dq_done, 0, (size_t)e.R * 4) == cudaSuccess;
+    ok = ok && cudaMemcpy(e.dT0, aesoff_T0_table(), 256 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+    if (!ok) {
+        free_engine_memory(e);
+        return fail(AES_E_CUDA);
+    }
+
+    aesoff_params_t p;
+    memset(&p, 0, sizeof(p));
+    p.hring = e.hring;
+    p.hmail = e.hmail;
+    p.hctl = e.hctl;
+    p.dq = e.dq;
+    p.tmap = e.tmap;
+    p.counters = e.counters;
+    p.dq_done = e.dq_done;
+    p.dev_done_seq = e.dev_done_seq;
+    p.T0 = e.dT0;
+    p.R = e.R;
+    p.TM = e.TM;
+    p.chunk_rows = e.chunk_rows;
+    p.mode = AESOFF_MODE_PERSISTENT;
+    p.idle_exit_ms = o.idle_exit_ms;
+    p.first_seq = e.first_seq;
+    if (aesoff_launch_engine(&p, e.n_ctas, e.stream) != 0) {
+        free_engine_memory(e);
+        return fail(AES_E_CUDA);
+    }
+    g_kernel_launches.fetch_add(1);
+    /* wait until the dispatcher warp is really polling (bounded) */
+    const uint64_t t0 = now_ns();
+    while (__atomic_load_n(&e.hctl[AESOFF_CTL_ALIVE], __ATOMIC_ACQUIRE) == 0u) {
+        if (now_ns() - t0 > 20ull * 1000000000ull || cudaStreamQuery(e.stream) != cudaErrorNotReady) {
+            __atomic_store_n(&e.hctl[AESOFF_CTL_STOP], 1u, __ATOMIC_RELEASE);
+            free_engine_memory(e);
+            return fail(AES_E_CUDA);
+        }
+        CPU_RELAX();
+    }
+    e.running.store(1, std::memory_order_release);
+    return AES_OK;
+}
+
+extern "C" int aes_engine_stop(void)
+{
+    std::lock_guard<std::mutex> lk(g_lifecycle);
+    Engine &e = g_eng;
+    if (!e.running.load()) return fail(AES_E_STOPPED);
+    /* no new submissions from here on */
+    e.running.store(2, std::memory_order_release);
+    int rc = AES_OK;
+    /* drain: every accepted request completes (unless the kernel died) */
+    const uint64_t last = e.next_seq.load();
+    for (uint64_t s = (last > e.first_seq + e.R) ? last - e.R : e.first_seq; s < last; ++s) {
+        const uint64_t t0 = now_ns();
+        while (__atomic_load_n(&e.hmail[(s - 1) & e.Rm], __ATOMIC_ACQUIRE) < s) {
+            /* a producer that claimed s has published it before submit returned, so this ends */
+            if (engine_dead(e) || now_ns() - t0 > 60ull * 1000000000ull) {
+                rc = AES_E_STOPPED;
+                break;
+            }
+            CPU_RELAX();
+        }
+        if (rc != AES_OK) break;
+    }
+    __atomic_store_n(&e.hctl[AESOFF_CTL_STOP], 1u, __ATOMIC_RELEASE);
+    if (cudaStreamSynchronize(e.stream) != cudaSuccess) rc = AES_E_CUDA;
+    free_engine_memory(e);
+    e.running.store(0, std::memory_order_release);
+    if (rc != AES_OK) return fail(rc);
+    return AES_OK;
+}
+
+extern "C" int aes_engine_info(aes_engine_info_t *out)
+{
+    if (!out) return fail(AES_E_INVAL);
+    memset(out, 0, sizeof(*out));
+    Engine &e = g_eng;
+    out->running = e.running.load() == 1 && e.hctl && !engine_dead(e);
+    out->device = e.device;
+    out->sm_count = e.sm_count;
+    out->n_ctas = e.n_ctas;
+    out->threads_per_cta = AESOFF_CTA_THREADS;
+    out->groups_per_cta = AESOFF_GROUPS_PER_CTA;
+    out->ring_slots = e.R;
+    out->chunk_rows = e.chunk_rows;
+    out->smem_bytes_per_cta = AESOFF_SMEM_BYTES;
+    const uint64_t next = e.next_seq.load();
+    out->submitted = next - 1;
+    uint64_t pending = 0;
+    if (e.running.load() && e.hmail) {
+        for (uint64_t s = (next > e.first_seq + e.R) ? next - e.R : e.first_seq; s < next; ++s)
+            if (__atomic_load_n(&e.hmail[(s - 1) & e.Rm], __ATOMIC_ACQUIRE) < s) ++pending;
+    }
+    out->completed = out->submitted - pending;
+    out->kernel_launches = g_kernel_launches.load();
+    return AES_OK;
+}
+
+/* ============================================================================================ */
+/* submit / poll / wait (steps a2, a7)                                                          */
+/* ============================================================================================ */
+extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], const void *src, void *dst,
+                                       size_t len)
+{
+    Engine &e = g_eng;
+    if (!ctx || !nonce) {
+        fail(AES_E_INVAL);
+        return 0;
+    }
+    const int rc = check_buffers(src, dst, len);
+    if (rc != AES_OK) {
+        fail(rc);
+        return 0;
+    }
+    if (e.running.load(std::memory_order_acquire) != 1 || engine_dead(e)) {
+        fail(AES_E_STOPPED);
+        return 0;
+    }
+    /* claim the next sequence number, but only if its slot has been vacated */
+    uint64_t s = e.next_seq.load(std::memory_order_acquire);
+    for (;;) {
+        if (s - e.first_seq >= e.R &&
+            __atomic_load_n(&e.hmail[(s - 1) & e.Rm], __ATOMIC_ACQUIRE) < s - e.R) {
+            fail(AES_E_AGAIN);
+            return 0;
+        }
+        if (e.next_seq.compare_exchange_weak(s, s + 1, std::memory_order_acq_rel)) break;
+    }
+    aesoff_host_slot_t *slot = &e.hring[(s - 1) & e.Rm];
+    memcpy(slot->rk, ctx->rk, sizeof(slot->rk));
+    memcpy(slot->icb, nonce, 16);
+    slot->src = (uint64_t)(uintptr_t)src;
+    slot->dst = (uint64_t)(uintptr_t)dst;
+    slot->len = (uint64_t)len;
+    slot->nr = (uint32_t)ctx->nr;
+    slot->flags = 0;
+    __atomic_store_n(&slot->seq, s, __ATOMIC_RELEASE);
+    return (aes_handle_t)s;
+}
+
+extern "C" int aes_poll(aes_handle_t h)
+{
+    Engine &e = g_eng;
+    if (h == 0 || h >= e.next_seq.load(std::memory_order_acquire)) return fail(AES_E_INVAL);
+    if (h < e.first_seq || !e.running.load(std::memory_order_acquire)) return 1; /* a stop drains everything */
+    if (__atomic_load_n(&e.hmail[(h - 1) & e.Rm], __ATOMIC_ACQUIRE) >= h) return 1;
+    if (engine_dead(e)) {
+        /* the exit path of the kernel cannot overtake a completion it already signalled */
+        if (__atomic_load_n(&e.hmail[(h - 1) & e.Rm], __ATOMIC_ACQUIRE) >= h) return 1;
+        return fail(AES_E_STOPPED);
+    }
+    return 0;
+}
+
+extern "C" int aes_wait(aes_handle_t h, uint64_t timeout_ns)
+{
+    const uint64_t t0 = now_ns();
+    for (uint32_t spins = 0;; ++spins) {
+        const int r = aes_poll(h);
+        if (r == 1) return AES_OK;
+        if (r < 0) return r;
+        if ((spins & 63u) == 63u && timeout_ns != UINT64_MAX && now_ns() - t0 > timeout_ns) return fail(AES_E_TIMEOUT);
+        CPU_RELAX();
+    }
+}
+
+/* ============================================================================================ */
+/* pinned host memory                                                                            */
+/* ============================================================================================ */
+extern "C" void *aes_host_alloc(size_t bytes)
+{
+    void *p = nullptr;
+    if (cudaHostAlloc(&p, bytes ? bytes : 1, cudaHostAllocMapped | cudaHostAllocPortable) != cudaSuccess) {
+        cudaGetLastError();
+        fail(AES_E_CUDA);
+        return nullptr;
+    }
+    return p;
+}
+extern "C" void aes_host_free(void *p)
+{
+    if (p) cudaFreeHost(p);
+}
+
+/* ============================================================================================ */
+/* launch backend: the paper's mechanism (own stream + event)                      */
+/* ============================================================================================ */
+namespace {
+struct LaunchCtx {
+    std::mutex mu;
+    int device = -1;
+    size_t cap_req = 0, cap_tickets = 0; /* capacities (power of two) */
+    aesoff_dev_desc_t *dq = nullptr;
+    uint64_t *tmap = nullptr, *counters = nullptr, *dev_done_seq = nullptr;
+    uint32_t *dq_done = nullptr, *dT0 = nullptr;
+    uint8_t *stage = nullptr; /* pinned */
+    size_t stage_bytes = 0;
+    cudaEvent_t stage_free = nullptr;
+    bool stage_busy = false;
+};
+LaunchCtx g_lc;
+
+size_t pow2_at_least(size_t x)
+{
+    size_t p = 64;
+    while (p < x) p <<= 1;
+    return p;
+}
+} /* namespace */
+
+extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonces, const void *const *srcs,
+                                    void *const *dsts, const size_t *lens, size_t n, int device, void *cuda_stream,
+                                    uint32_t chunk_rows)
+{
+    if (n == 0) return AES_OK;
+    if (!ctxs || !nonces || !srcs || !dsts || !lens) return fail(AES_E_INVAL);
+    if (chunk_rows == 0) chunk_rows = 4;
+    if (chunk_rows > 64) return fail(AES_E_INVAL);
+    if (g_eng.running.load()) return fail(AES_E_BUSY);
+    for (size_t i = 0; i < n; ++i) {
+        if (!ctxs[i]) return fail(AES_E_INVAL);
+        const int rc = check_buffers(srcs[i], dsts[i], lens[i]);
+        if (rc != AES_OK) return fail(rc);
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(AES_E_CUDA);
+    if (cudaSetDevice(device) != cudaSuccess) return fail(AES_E_CUDA);
+    int sms = 0, major = 0;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
+    cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
+    if (major != 10) return fail(AES_E_CUDA);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    LaunchCtx &L = g_lc;
+    std::lock_guard<std::mutex> lk(L.mu);
+
+    /* geometry first: how many tickets in all */
+    const size_t R = pow2_at_least(n);
+    std::vector<uint64_t> rows(n);
+    std::vector<uint32_t> crows(n), nch(n);
+    uint64_t total = 0;
+    for (size_t i = 0; i < n; ++i) {
+        request_geometry(lens[i], nonces[16 * i + 15], chunk_rows, 1u << 24, &rows[i], &crows[i], &nch[i]);
+        total += nch[i];
+    }
+    if (total >= (1ull << 30)) return fail(AES_E_INVAL);
+    const size_t TM = pow2_at_least((size_t)total);
+
+    /* (re)allocate device queue and pinned staging */
+    if (L.device != device || L.cap_req < R || L.cap_tickets < TM) {
+        if (L.stage_busy) cudaEventSynchronize(L.stage_free);
+        L.stage_busy = false;
+        if (L.dq) cudaFree(L.dq);
+        if (L.tmap) cudaFree(L.tmap);
+        if (L.counters) cudaFree(L.counters);
+        if (L.dev_done_seq) cudaFree(L.dev_done_seq);
+        if (L.dq_done) cudaFree(L.dq_done);
+        if (L.dT0) cudaFree(L.dT0);
+        if (L.stage) cudaFreeHost(L.stage);
+        if (!L.stage_free) cudaEventCreateWithFlags(&L.stage_free, cudaEventDisableTiming);
+        L.dq = nullptr;
+        L.cap_req = R > L.cap_req ? R : L.cap_req;
+        L.cap_tickets = TM > L.cap_tickets ? TM : L.cap_tickets;
+        L.stage_bytes = L.cap_req * sizeof(aesoff_dev_desc_t) + L.cap_tickets * 8 + AESOFF_CNT_WORDS * 8;
+        bool ok = true;
+        ok = ok && cudaMalloc((void **)&L.dq, L.cap_req * sizeof(aesoff_dev_desc_t)) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.tmap, L.cap_tickets * 8) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.counters, AESOFF_CNT_WORDS * 8) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.dev_done_seq, L.cap_req * 8) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.dq_done, L.cap_req * 4) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.dT0, 256 * 4) == cudaSuccess;
+        ok = ok && cudaHostAlloc((void **)&L.stage, L.stage_bytes, cudaHostAllocDefault) == cudaSuccess;
+        ok = ok && cudaMemcpy(L.dT0, aesoff_T0_table(), 256 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+        ok = ok && cudaMemset(L.dq_done, 0, L.cap_req * 4) == cudaSuccess;
+        ok = ok && cudaMemset(L.dev_done_seq, 0, L.cap_req * 8) == cudaSuccess;
+        if (!ok) {
+            cudaGetLastError();
+            L.device = -1;
+            L.cap_req = L.cap_tickets = 0;
+            return fail(AES_E_NOMEM);
+        }
+        L.device = device;
+    }
+    /* the previous call's copies must have left the staging buffer */
+    if (L.stage_busy) {
+        cudaEventSynchronize(L.stage_free);
+        L.stage_busy = false;
+    }
+    aesoff_dev_desc_t *hd = reinterpret_cast<aesoff_dev_desc_t *>(L.stage);
+    uint64_t *ht = reinterpret_cast<uint64_t *>(L.stage + L.cap_req * sizeof(aesoff_dev_desc_t));
+    uint64_t *hc = ht + L.cap_tickets;
+    uint64_t t = 0;
+    for (size_t i = 0; i < n; ++i) {
+        aesoff_dev_desc_t &d = hd[i];
+        memcpy(d.rk, ctxs[i]->rk, sizeof(d.rk));
+        memcpy(d.icb, nonces + 16 * i, 16);
+        d.src = (uint64_t)(uintptr_t)srcs[i];
+        d.dst = (uint64_t)(uintptr_t)dsts[i];
+        d.len = (uint64_t)lens[i];
+        d.nr = (uint32_t)ctxs[i]->nr;
+        d.flags = 0;
+        d.nchunks = nch[i];
+        d.chunk_rows = crows[i];
+        d.seq = i + 1;
+        d.rows = rows[i];
+        d.pad = t;
+        for (uint32_t c = 0; c < nch[i]; ++c) ht[t + c] = ((uint64_t)(i + 1) << AESOFF_TICKET_CHUNK_BITS) | c;
+        t += nch[i];
+    }
+    memset(hc, 0, AESOFF_CNT_WORDS * 8);
+    hc[AESOFF_CNT_PUBLISHED] = total;
+
+    bool ok = true;
+    ok = ok && cudaMemcpyAsync(L.dq, hd, n * sizeof(aesoff_dev_desc_t), cudaMemcpyHostToDevice, stream) == cudaSuccess;
+    if (total)
+        ok = ok && cudaMemcpyAsync(L.tmap, ht, (size_t)total * 8, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(L.counters, hc, AESOFF_CNT_WORDS * 8, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+    ok = ok && cudaEventRecord(L.stage_free, stream) == cudaSuccess;
+    L.stage_busy = true;
+    if (!ok) {
+        cudaGetLastError();
+        return fail(AES_E_CUDA);
+    }
+    if (total == 0) return AES_OK;
+
+    aesoff_params_t p;
+    memset(&p, 0, sizeof(p));
+    p.dq = L.dq;
+    p.tmap = L.tmap;
+    p.counters = L.counters;
+    p.dq_done = L.dq_done;
+    p.dev_done_seq = L.dev_done_seq;
+    p.T0 = L.dT0;
+    p.drain_total = total;
+    p.R = (uint32_t)R;
+    p.TM = (uint32_t)L.cap_tickets;
+    p.chunk_rows = chunk_rows;
+    p.mode = AESOFF_MODE_DRAIN;
+    p.first_seq = 1;
+    uint64_t ctas = (total + AESOFF_GROUPS_PER_CTA - 1) / AESOFF_GROUPS_PER_CTA;
+    if (ctas > (uint64_t)sms) ctas = (uint64_t)sms;
+    if (aesoff_launch_engine(&p, (int)ctas, stream) != 0) return fail(AES_E_CUDA);
+    g_kernel_launches.fetch_add(1);
+    return AES_OK;
+}
+
+/* ============================================================================================ */
+/* closed-loop executor (PAPER.md:127-135 worker loop; "50 concurrent clients")      */
+/* ============================================================================================ */
+extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res, double *lat_ns)
+{
+    if (!spec || !res || !spec->nonces || !spec->srcs || !spec->dsts || !spec->lens) return fail(AES_E_INVAL);
+    if (!spec->keys && !spec->ctx) return fail(AES_E_INVAL);
+    if (spec->keys && !spec->keybits) return fail(AES_E_INVAL);
+    if (spec->n == 0 || spec->window == 0) return fail(AES_E_INVAL);
+    Engine &e = g_eng;
+    if (e.running.load() != 1) return fail(AES_E_STOPPED);
+    const uint64_t repeat = spec->repeat ? spec->repeat : 1;
+    const uint64_t total = (uint64_t)spec->n * repeat;
+    const uint32_t window = spec->window > e.R ? e.R : spec->window;
+
+    struct Fly {
+        aes_handle_t h;
+        uint64_t t_submit;
+        uint64_t index;
+    };
+    std::vector<Fly> fly(window);
+    uint32_t n_fly = 0;
+    uint64_t next = 0, done = 0, bytes = 0;
+    memset(res, 0, sizeof(*res));
+
+    const uint64_t t_begin = now_ns();
+    while (done < total) {
+        /* submit until the window is full */
+        while (n_fly < window && next < total) {
+            const size_t i = (size_t)(next % spec->n);
+            aes_ctx_t *ctx = spec->ctx;
+            if (spec->keys) {
+                ctx = aes_ctx_create(spec->keys + 32 * i, spec->keybits[i]);
+                if (!ctx) return t_last_error;
+            }
+            const uint64_t ts = now_ns();
+            const aes_handle_t h = aes_ctr_submit(ctx, spec->nonces + 16 * i, spec->srcs[i], spec->dsts[i], spec->lens[i]);
+            if (spec->keys) aes_ctx_destroy(ctx);
+            if (h == 0) {
+                if (t_last_error == AES_E_AGAIN) {
+                    ++res->ring_full_spins;
+                    break;
+                }
+                return t_last_error;
+            }
+            fly[n_fly++] = Fly{h, ts, next};
+            if (n_fly > res->max_in_flight) res->max_in_flight = n_fly;
+            ++next;
+        }
+        /* poll everything in flight; compact the array as completions are seen */
+        uint32_t k = 0;
+        while (k < n_fly) {
+            const int r = aes_poll(fly[k].h);
+            if (r == 1) {
+                if (lat_ns) lat_ns[fly[k].index] = (double)(now_ns() - fly[k].t_submit);
+                bytes += spec->lens[fly[k].index % spec->n];
+                ++done;
+                fly[k] = fly[--n_fly];
+            } else if (r < 0) {
+                return r;
+            } else {
+                ++k;
+            }
+        }
+    }
+    res->elapsed_ns = now_ns() - t_begin;
+    res->bytes = bytes;
+    res->requests = done;
+    return AES_OK;
+}

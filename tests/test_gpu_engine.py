@@ -1,0 +1,296 @@
+"""-m gpu parity and behaviour of the persistent engine: submission ring -> dispatcher warp ->
+worker groups -> completion mailbox (steps a2, a3, a7 of SURVEY.md section 8(a)), against the
+oracle, byte for byte.
+
+While the engine runs, a device-wide synchronisation would block on the persistent kernel, so these
+tests only use host<->device copies (no torch kernels) and stream-level synchronisation.
+"""
+import threading
+
+import numpy as np
+import pytest
+
+from paper_2607_02630_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2607_02630_b200.binding as B
+    from tests import gpu_util as G
+
+    torch = G.torch_cuda()
+    torch.zeros(1, device="cuda:0")  # CUDA context + torch's first kernels before the engine occupies the SMs
+    torch.cuda.synchronize()
+    B.aes_engine_start(0, idle_exit_ms=60000)
+    yield B
+    B.aes_engine_stop()
+
+
+def _submit_all(P, reqs, in_place=False, host=False):
+    """reqs: (key, icb, ndarray).  Submits everything (spinning on ring-full), waits, returns outputs."""
+    from tests import gpu_util as G
+
+    ctxs, srcs, dsts, hs = {}, [], [], []
+    for key, icb, data in reqs:
+        if key not in ctxs:
+            ctxs[key] = P.aes_ctx_create(key)
+        s = G.to_device(data) if len(data) else G.device_empty(0)
+        srcs.append(s)
+        dsts.append(s if in_place else G.device_empty(len(data)))
+    G.stream_sync()
+    for (key, icb, data), s, d in zip(reqs, srcs, dsts):
+        while True:
+            try:
+                hs.append(P.aes_ctr_submit(ctxs[key], icb, s.data_ptr(), d.data_ptr(), len(data)))
+                break
+            except P.AesOffError as e:
+                if e.code != P.AES_E_AGAIN:
+                    raise
+    for h in hs:
+        P.aes_wait(h, 20_000_000_000)
+        assert P.aes_poll(h) is True
+    outs = [d.cpu().numpy()[: len(x)] for d, (_, _, x) in zip(dsts, reqs)]
+    for c in ctxs.values():
+        P.aes_ctx_destroy(c)
+    return outs
+
+
+def _check(P, reqs, **kw):
+    from tests import gpu_util as G
+
+    outs = _submit_all(P, reqs, **kw)
+    wants = G.oracle_many([(k, i, d) for k, i, d in reqs])
+    for n, (got, want) in enumerate(zip(outs, wants)):
+        bad = G.first_mismatch(got, want)
+        assert bad == -1, "request %d (len %d, keybits %d, icb %s): first mismatch at byte %d" % (
+            n, len(reqs[n][2]), 8 * len(reqs[n][0]), reqs[n][1].hex(), bad)
+
+
+def test_engine_info(P):
+    info = P.aes_engine_info()
+    assert info["running"] == 1 and info["n_ctas"] == info["sm_count"] >= 100
+    assert info["kernel_launches"] >= 1
+
+
+def test_config1_single_request(P):
+    w = workloads.config1()
+    _check(P, [(w.key_of(0), w.icb_of(0), w.payload(0))])
+
+
+def test_lengths_and_carries(P):
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7000]))
+    reqs = []
+    for keylen in (16, 32):
+        key = rng.bytes(keylen)
+        for n in (0, 1, 15, 16, 17, 4095, 4096, 4097, 16385, 65536 + 5, (1 << 20) + 5):
+            reqs.append((key, rng.bytes(8) + bytes(8), np.frombuffer(rng.bytes(n), dtype=np.uint8)))
+        for icb in workloads.edge_icbs():
+            reqs.append((key, icb, np.frombuffer(rng.bytes(16 * 600 + 3), dtype=np.uint8)))
+    _check(P, reqs)
+
+
+def test_config2_shape_64_in_flight(P):
+    """configs[1] at reduced count: 64 x 1 MiB AES-128, one key, distinct nonces, all 64 in flight."""
+    w = workloads.config2(n=64)
+    _check(P, [(w.key_of(i), w.icb_of(i), w.payload(i)) for i in range(w.n)])
+
+
+def test_config3_shape_sampled(P):
+    """configs[2] at reduced count: 16 x 8 MiB AES-256 in flight; sampled 64 KiB windows per request
+    (first, last, 2 random) through oracle_ctr_at."""
+    from tests import gpu_util as G
+
+    w = workloads.config3(n=16)
+    ctx = P.aes_ctx_create(w.key_of(0))
+    srcs = [G.to_device(w.payload(i)) for i in range(w.n)]
+    dsts = [G.device_empty(int(w.length[i])) for i in range(w.n)]
+    G.stream_sync()
+    hs = [P.aes_ctr_submit(ctx, w.icb_of(i), srcs[i].data_ptr(), dsts[i].data_ptr(), int(w.length[i]))
+          for i in range(w.n)]
+    for h in hs:
+        P.aes_wait(h, 20_000_000_000)
+    P.aes_ctx_destroy(ctx)
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7100]))
+    W = 64 << 10
+    jobs, gots, tags = [], [], []
+    for i in range(w.n):
+        n = int(w.length[i])
+        src_h = w.payload(i)
+        out_h = dsts[i].cpu().numpy()
+        for s0 in [0, n - W] + [int(x) * 16 for x in rng.integers(0, (n - W) // 16, size=2)]:
+            jobs.append((w.key_of(i), w.icb_of(i), src_h[s0:s0 + W], s0 // 16))
+            gots.append(out_h[s0:s0 + W])
+            tags.append((i, s0))
+    for tag, got, want in zip(tags, gots, G.oracle_many(jobs)):
+        assert G.first_mismatch(got, want) == -1, "request %d window at %d" % tag
+
+
+def test_config4_mix_per_request_keys_native_loop(P):
+    """configs[3] at reduced count through the native closed loop: 1,500 requests, sizes log-uniform
+    1-64 KiB with 0-15 B tails, per-request AES-128/256 keys expanded inside the loop, fully random
+    ICBs, 256 in flight.  Every byte checked."""
+    from tests import gpu_util as G
+
+    w = workloads.config4(n=1500)
+    srcs = [G.to_device(w.payload(i)) for i in range(w.n)]
+    dsts = [G.device_empty(int(w.length[i])) for i in range(w.n)]
+    G.stream_sync()
+    keys = np.zeros((w.n, 32), dtype=np.uint8)
+    keybits = np.zeros(w.n, dtype=np.int32)
+    for i in range(w.n):
+        k = w.key_of(i)
+        keys[i, : len(k)] = np.frombuffer(k, dtype=np.uint8)
+        keybits[i] = 8 * len(k)
+    r = P.aes_loop_run(w.icb, [s.data_ptr() for s in srcs], [d.data_ptr() for d in dsts], w.length,
+                       window=w.in_flight, keys=keys, keybits=keybits)
+    assert r["requests"] == w.n and r["bytes"] == w.total_bytes
+    assert r["max_in_flight"] <= w.in_flight
+    assert (r["lat_ns"] > 0).all()
+    wants = G.oracle_many([(w.key_of(i), w.icb_of(i), w.payload(i)) for i in range(w.n)])
+    for i in range(w.n):
+        got = dsts[i].cpu().numpy()[: int(w.length[i])]
+        assert G.first_mismatch(got, wants[i]) == -1, "request %d len %d" % (i, int(w.length[i]))
+
+
+def test_buffer_reuse_sees_fresh_data(P):
+    """The persistent kernel's L1 is never invalidated: a recycled src buffer must still be read
+    fresh (payload loads are L2-only).  Same buffers, new contents, 20 rounds, in place and not."""
+    from tests import gpu_util as G
+
+    torch = G.torch_cuda()
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7200]))
+    key, n = rng.bytes(16), 48 * 1024 + 7
+    ctx = P.aes_ctx_create(key)
+    src, dst = G.device_empty(n), G.device_empty(n)
+    from oracle import oracle as o
+
+    for it in range(20):
+        data = np.frombuffer(rng.bytes(n), dtype=np.uint8)
+        icb = rng.bytes(16)
+        src.copy_(torch.from_numpy(data))  # H2D memcpy, no kernel
+        G.stream_sync()
+        target = src if it % 2 else dst
+        h = P.aes_ctr_submit(ctx, icb, src.data_ptr(), target.data_ptr(), n)
+        P.aes_wait(h)
+        assert G.first_mismatch(target.cpu().numpy(), o.ctr(key, icb, data)) == -1, "round %d" % it
+    P.aes_ctx_destroy(ctx)
+
+
+def test_host_resident_payload_zero_copy(P):
+    """src/dst in pinned host memory (aes_host_alloc): the kernel reads and writes over PCIe; once
+    aes_poll is true the host sees every byte."""
+    from oracle import oracle as o
+
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7300]))
+    for keylen, n in ((16, 4096), (32, 100003), (16, 1 << 20)):
+        key, icb = rng.bytes(keylen), rng.bytes(16)
+        ps, pd = P.aes_host_alloc(n), P.aes_host_alloc(n)
+        hs, hd = P.host_view(ps, n), P.host_view(pd, n)
+        hs[:] = np.frombuffer(rng.bytes(n), dtype=np.uint8)
+        hd[:] = 0
+        ctx = P.aes_ctx_create(key)
+        h = P.aes_ctr_submit(ctx, icb, ps, pd, n)
+        P.aes_wait(h)
+        want = o.ctr(key, icb, hs)
+        assert hd.tobytes() == want
+        P.aes_ctx_destroy(ctx)
+        del hs, hd
+        # freeing pinned memory synchronises the device: keep it until the engine stops (leak in test)
+
+
+def test_ring_full_then_drains(P):
+    """More submissions than ring slots: submit returns AES_E_AGAIN (never blocks), and every
+    accepted request still completes with the right bytes."""
+    from oracle import oracle as o
+    from tests import gpu_util as G
+
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7400]))
+    slots = P.aes_engine_info()["ring_slots"]
+    key = rng.bytes(16)
+    ctx = P.aes_ctx_create(key)
+    n = 8 << 20
+    big = G.to_device(np.frombuffer(rng.bytes(n), dtype=np.uint8))
+    sink = G.device_empty(n)
+    small_src = G.to_device(np.frombuffer(rng.bytes(256), dtype=np.uint8))
+    small_dst = G.device_empty(256)
+    G.stream_sync()
+    handles, again = [], 0
+    for i in range(slots + 64):
+        try:
+            handles.append(P.aes_ctr_submit(ctx, bytes(16), big.data_ptr(), sink.data_ptr(), n))
+        except P.AesOffError as e:
+            assert e.code == P.AES_E_AGAIN
+            again += 1
+    assert len(handles) + again == slots + 64
+    icb = rng.bytes(16)
+    while True:
+        try:
+            hs = P.aes_ctr_submit(ctx, icb, small_src.data_ptr(), small_dst.data_ptr(), 256)
+            break
+        except P.AesOffError as e:
+            assert e.code == P.AES_E_AGAIN
+    for h in handles + [hs]:
+        P.aes_wait(h, 60_000_000_000)
+    assert small_dst.cpu().numpy().tobytes() == o.ctr(key, icb, small_src.cpu().numpy())
+    assert sink.cpu().numpy()[:4096].tobytes() == o.ctr(key, bytes(16), big[:4096].cpu().numpy())
+    P.aes_ctx_destroy(ctx)
+
+
+def test_many_threads_submit(P):
+    """aes_ctr_submit from 8 executor threads at once (PAPER.md:350 '32-thread executor')."""
+    from tests import gpu_util as G
+
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7500]))
+    key = rng.bytes(32)
+    ctx = P.aes_ctx_create(key)
+    per, nthreads = 40, 8
+    reqs = [(rng.bytes(16), np.frombuffer(rng.bytes(int(rng.integers(1, 20000))), dtype=np.uint8))
+            for _ in range(per * nthreads)]
+    srcs = [G.to_device(d) for _, d in reqs]
+    dsts = [G.device_empty(len(d)) for _, d in reqs]
+    G.stream_sync()
+    errors = []
+
+    def run(t):
+        try:
+            hs = []
+            for i in range(t * per, (t + 1) * per):
+                hs.append(P.aes_ctr_submit(ctx, reqs[i][0], srcs[i].data_ptr(), dsts[i].data_ptr(), len(reqs[i][1])))
+            for h in hs:
+                P.aes_wait(h)
+        except Exception as e:  # noqa: BLE001
+            errors.append(e)
+
+    ts = [threading.Thread(target=run, args=(t,)) for t in range(nthreads)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    assert not errors
+    wants = G.oracle_many([(key, icb, d) for icb, d in reqs])
+    for i, want in enumerate(wants):
+        assert G.first_mismatch(dsts[i].cpu().numpy()[: len(reqs[i][1])], want) == -1, "request %d" % i
+    P.aes_ctx_destroy(ctx)
+
+
+def test_errors_and_handles(P):
+    from tests import gpu_util as G
+
+    ctx = P.aes_ctx_create(bytes(16))
+    buf = G.device_empty(4096)
+    p = buf.data_ptr()
+    for args, code in (((ctx, bytes(16), p + 4, p, 64), P.AES_E_ALIGN),
+                       ((ctx, bytes(16), p, p + 32, 64), P.AES_E_OVERLAP),
+                       ((0, bytes(16), p, p, 64), P.AES_E_INVAL)):
+        with pytest.raises(P.AesOffError) as e:
+            P.aes_ctr_submit(*args)
+        assert e.value.code == code
+    with pytest.raises(P.AesOffError) as e:
+        P.aes_poll(1 << 60)  # never issued
+    assert e.value.code == P.AES_E_INVAL
+    with pytest.raises(P.AesOffError) as e:
+        P.aes_ctr_launch_batch([ctx], bytes(16), [p], [p], [64])  # engine is running
+    assert e.value.code == P.AES_E_BUSY
+    h = P.aes_ctr_submit(ctx, bytes(16), 0, 0, 0)  # len 0: completes, touches nothing
+    P.aes_wait(h)
+    P.aes_ctx_destroy(ctx)

@@ -1,0 +1,163 @@
+"""-m gpu parity, launch backend (aes_ctr_launch_batch): the CUDA path against the oracle,
+byte for byte (bit-exact: AES-CTR has one correct output).
+
+The launch backend runs exactly the worker code of the persistent engine from an ordinary kernel
+launch, so these cases pin the arithmetic (counter blocks, rounds, tails, chunking) independently of
+the ring/mailbox machinery, which tests/test_gpu_engine.py covers.
+"""
+import numpy as np
+import pytest
+
+from paper_2607_02630_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2607_02630_b200.binding as B
+
+    return B
+
+
+def _run_batch(P, reqs, chunk_rows=0, in_place=False):
+    """reqs: list of (key, icb, payload ndarray).  Returns list of output ndarrays."""
+    from tests import gpu_util as G
+
+    ctxs = {}
+    srcs, dsts, handles = [], [], []
+    for key, icb, data in reqs:
+        if key not in ctxs:
+            ctxs[key] = P.aes_ctx_create(key)
+        s = G.to_device(data) if len(data) else G.device_empty(0)
+        d = s if in_place else G.device_empty(len(data))
+        srcs.append(s)
+        dsts.append(d)
+    G.stream_sync()
+    P.aes_ctr_launch_batch([ctxs[k] for k, _, _ in reqs], b"".join(icb for _, icb, _ in reqs),
+                           [s.data_ptr() for s in srcs], [d.data_ptr() for d in dsts],
+                           [len(x) for _, _, x in reqs], cuda_stream=0, chunk_rows=chunk_rows)
+    G.torch_cuda().cuda.synchronize()  # no persistent engine in this module: a device sync is fine
+    outs = [d.cpu().numpy()[: len(x)] for d, (_, _, x) in zip(dsts, reqs)]
+    for c in ctxs.values():
+        P.aes_ctx_destroy(c)
+    return outs
+
+
+def _check(P, reqs, **kw):
+    from tests import gpu_util as G
+
+    outs = _run_batch(P, reqs, **kw)
+    wants = G.oracle_many([(k, i, d) for k, i, d in reqs])
+    for n, (got, want) in enumerate(zip(outs, wants)):
+        bad = G.first_mismatch(got, want)
+        assert bad == -1, "request %d (len %d, keybits %d, icb %s): first mismatch at byte %d" % (
+            n, len(reqs[n][2]), 8 * len(reqs[n][0]), reqs[n][1].hex(), bad)
+
+
+def test_config1_aes128_64KiB(P):
+    w = workloads.config1()
+    _check(P, [(w.key_of(0), w.icb_of(0), w.payload(0))])
+
+
+@pytest.mark.parametrize("keylen", [16, 32])
+def test_lengths_tails_and_tiles(P, keylen):
+    """Empty, sub-block, block +-1, row (4 KiB) +-1, chunk (16 KiB) +-1, several chunks + ragged tail."""
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 1000 + keylen]))
+    key = rng.bytes(keylen)
+    lens = [0, 1, 15, 16, 17, 31, 32, 33, 255, 256, 4095, 4096, 4097, 4111, 16383, 16384, 16385,
+            65536 + 5, 3 * 16384 + 16 * 77 + 9, (1 << 20) + 5]
+    reqs = []
+    for n in lens:
+        icb = rng.bytes(8) + bytes(8)
+        reqs.append((key, icb, np.frombuffer(rng.bytes(n), dtype=np.uint8)))
+    _check(P, reqs)
+
+
+@pytest.mark.parametrize("keylen", [16, 32])
+def test_counter_carries(P, keylen):
+    """R4: the counter is a 128-bit big-endian integer; carries out of the low 8/32/64/128 bits, both
+    on the first increment and in the middle of a chunk, and ICBs whose last byte is not zero (rows
+    are aligned on that byte)."""
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 2000 + keylen]))
+    key = rng.bytes(keylen)
+    reqs = []
+    for icb in workloads.edge_icbs():
+        for n in (16 * 600 + 3, 16 * 70, 40000):
+            reqs.append((key, icb, np.frombuffer(rng.bytes(n), dtype=np.uint8)))
+    for last in (1, 31, 32, 33, 128, 254, 255):
+        icb = rng.bytes(15) + bytes([last])
+        for n in (5, 16 * (256 - last), 16 * (256 - last) + 1, 16 * 300 + 7, 70001):
+            reqs.append((key, icb, np.frombuffer(rng.bytes(n), dtype=np.uint8)))
+    _check(P, reqs)
+
+
+@pytest.mark.parametrize("chunk_rows", [1, 2, 16, 64])
+def test_chunk_sizes(P, chunk_rows):
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 3000 + chunk_rows]))
+    reqs = []
+    for keylen, n in ((16, 300000 + 7), (32, 1 << 19), (16, 4096 * 64 + 16), (32, 100)):
+        reqs.append((rng.bytes(keylen), rng.bytes(16), np.frombuffer(rng.bytes(n), dtype=np.uint8)))
+    _check(P, reqs, chunk_rows=chunk_rows)
+
+
+def test_in_place_and_mixed_keys(P):
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 4000]))
+    reqs = [(rng.bytes(16 if i % 2 else 32), rng.bytes(16), np.frombuffer(rng.bytes(1000 * i + i), dtype=np.uint8))
+            for i in range(1, 40)]
+    _check(P, reqs, in_place=True)
+
+
+def test_decrypt_is_encrypt(P):
+    """CTR is an involution (SP 800-38A 6.5): running the output through again returns the input."""
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 5000]))
+    key, icb = rng.bytes(32), rng.bytes(16)
+    data = np.frombuffer(rng.bytes(123457), dtype=np.uint8)
+    (ct,) = _run_batch(P, [(key, icb, data)])
+    (pt,) = _run_batch(P, [(key, icb, ct)])
+    assert np.array_equal(pt, data) and not np.array_equal(ct, data)
+
+
+def test_large_request_sampled_windows(P):
+    """64 MiB AES-256 (the sweep's largest size): too long for the byte-level oracle in full, so check
+    sampled 64 KiB windows with oracle_ctr_at, always including the first and the last block."""
+    from tests import gpu_util as G
+
+    torch = G.torch_cuda()
+    n = 64 << 20
+    g = torch.Generator(device="cuda:0").manual_seed(workloads.SEED_BASE + 5)
+    src = torch.randint(0, 256, (n,), dtype=torch.uint8, device="cuda:0", generator=g)
+    dst = torch.empty_like(src)
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 6000]))
+    key, icb = rng.bytes(32), rng.bytes(16)
+    ctx = P.aes_ctx_create(key)
+    torch.cuda.synchronize()
+    P.aes_ctr_launch_batch([ctx], icb, [src.data_ptr()], [dst.data_ptr()], [n])
+    torch.cuda.synchronize()
+    P.aes_ctx_destroy(ctx)
+    W = 64 << 10
+    starts = [0, n - W] + [int(x) * 16 for x in rng.integers(0, (n - W) // 16, size=10)]
+    jobs, gots = [], []
+    for s0 in starts:
+        jobs.append((key, icb, src[s0:s0 + W].cpu().numpy(), s0 // 16))
+        gots.append(dst[s0:s0 + W].cpu().numpy())
+    for s0, got, want in zip(starts, gots, G.oracle_many(jobs)):
+        assert G.first_mismatch(got, want) == -1, "window at %d" % s0
+
+
+def test_errors_launch(P):
+    from tests import gpu_util as G
+
+    ctx = P.aes_ctx_create(bytes(16))
+    buf = G.device_empty(4096)
+    p = buf.data_ptr()
+    with pytest.raises(P.AesOffError) as e:
+        P.aes_ctr_launch_batch([ctx], bytes(16), [p + 1], [p + 1], [64])
+    assert e.value.code == P.AES_E_ALIGN
+    with pytest.raises(P.AesOffError) as e:
+        P.aes_ctr_launch_batch([ctx], bytes(16), [p], [p + 16], [64])
+    assert e.value.code == P.AES_E_OVERLAP
+    with pytest.raises(P.AesOffError) as e:
+        P.aes_ctr_launch_batch([0], bytes(16), [p], [p], [64])
+    assert e.value.code == P.AES_E_INVAL
+    P.aes_ctx_destroy(ctx)
