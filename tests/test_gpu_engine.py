@@ -18,7 +18,7 @@ pytestmark = pytest.mark.gpu
 @pytest.fixture(scope="module")
 def P():
     import paper_2607_02630_b200.binding as B
-    from tests import gpu_util as G
+    import gpu_util as G
 
     torch = G.torch_cuda()
     torch.zeros(1, device="cuda:0")  # CUDA context + torch's first kernels before the engine occupies the SMs
@@ -30,7 +30,7 @@ def P():
 
 def _submit_all(P, reqs, in_place=False, host=False):
     """reqs: (key, icb, ndarray).  Submits everything (spinning on ring-full), waits, returns outputs."""
-    from tests import gpu_util as G
+    import gpu_util as G
 
     ctxs, srcs, dsts, hs = {}, [], [], []
     for key, icb, data in reqs:
@@ -58,7 +58,7 @@ def _submit_all(P, reqs, in_place=False, host=False):
 
 
 def _check(P, reqs, **kw):
-    from tests import gpu_util as G
+    import gpu_util as G
 
     outs = _submit_all(P, reqs, **kw)
     wants = G.oracle_many([(k, i, d) for k, i, d in reqs])
@@ -100,7 +100,7 @@ def test_config2_shape_64_in_flight(P):
 def test_config3_shape_sampled(P):
     """configs[2] at reduced count: 16 x 8 MiB AES-256 in flight; sampled 64 KiB windows per request
     (first, last, 2 random) through oracle_ctr_at."""
-    from tests import gpu_util as G
+    import gpu_util as G
 
     w = workloads.config3(n=16)
     ctx = P.aes_ctx_create(w.key_of(0))
@@ -131,7 +131,7 @@ def test_config4_mix_per_request_keys_native_loop(P):
     """configs[3] at reduced count through the native closed loop: 1,500 requests, sizes log-uniform
     1-64 KiB with 0-15 B tails, per-request AES-128/256 keys expanded inside the loop, fully random
     ICBs, 256 in flight.  Every byte checked."""
-    from tests import gpu_util as G
+    import gpu_util as G
 
     w = workloads.config4(n=1500)
     srcs = [G.to_device(w.payload(i)) for i in range(w.n)]
@@ -157,7 +157,7 @@ def test_config4_mix_per_request_keys_native_loop(P):
 def test_buffer_reuse_sees_fresh_data(P):
     """The persistent kernel's L1 is never invalidated: a recycled src buffer must still be read
     fresh (payload loads are L2-only).  Same buffers, new contents, 20 rounds, in place and not."""
-    from tests import gpu_util as G
+    import gpu_util as G
 
     torch = G.torch_cuda()
     rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7200]))
@@ -204,7 +204,7 @@ def test_ring_full_then_drains(P):
     """More submissions than ring slots: submit returns AES_E_AGAIN (never blocks), and every
     accepted request still completes with the right bytes."""
     from oracle import oracle as o
-    from tests import gpu_util as G
+    import gpu_util as G
 
     rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7400]))
     slots = P.aes_engine_info()["ring_slots"]
@@ -240,7 +240,7 @@ def test_ring_full_then_drains(P):
 
 def test_many_threads_submit(P):
     """aes_ctr_submit from 8 executor threads at once (PAPER.md:350 '32-thread executor')."""
-    from tests import gpu_util as G
+    import gpu_util as G
 
     rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7500]))
     key = rng.bytes(32)
@@ -274,7 +274,7 @@ def test_many_threads_submit(P):
 
 
 def test_errors_and_handles(P):
-    from tests import gpu_util as G
+    import gpu_util as G
 
     ctx = P.aes_ctx_create(bytes(16))
     buf = G.device_empty(4096)

@@ -22,7 +22,7 @@ def P():
 
 def _run_batch(P, reqs, chunk_rows=0, in_place=False):
     """reqs: list of (key, icb, payload ndarray).  Returns list of output ndarrays."""
-    from tests import gpu_util as G
+    import gpu_util as G
 
     ctxs = {}
     srcs, dsts, handles = [], [], []
@@ -45,7 +45,7 @@ def _run_batch(P, reqs, chunk_rows=0, in_place=False):
 
 
 def _check(P, reqs, **kw):
-    from tests import gpu_util as G
+    import gpu_util as G
 
     outs = _run_batch(P, reqs, **kw)
     wants = G.oracle_many([(k, i, d) for k, i, d in reqs])
@@ -121,7 +121,7 @@ def test_decrypt_is_encrypt(P):
 def test_large_request_sampled_windows(P):
     """64 MiB AES-256 (the sweep's largest size): too long for the byte-level oracle in full, so check
     sampled 64 KiB windows with oracle_ctr_at, always including the first and the last block."""
-    from tests import gpu_util as G
+    import gpu_util as G
 
     torch = G.torch_cuda()
     n = 64 << 20
@@ -146,7 +146,7 @@ def test_large_request_sampled_windows(P):
 
 
 def test_errors_launch(P):
-    from tests import gpu_util as G
+    import gpu_util as G
 
     ctx = P.aes_ctx_create(bytes(16))
     buf = G.device_empty(4096)
