@@ -1,0 +1,459 @@
+#!/usr/bin/env python
+"""bench.py -- the benchmark contract for the AES-CTR offload engine.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--backend engine|launch] [--workload c2|c3] [--no-extras]
+
+A *step* is one pass of the whole hot path (submit -> dispatch -> counter
+blocks -> cipher -> XOR/store -> completion) over one batch of synthetic input.  At N = 1 the batch
+is BASELINE.json configs[1], the configuration the metric is quoted on: 1,000 requests of 1 MiB,
+AES-128-CTR, one shared key, distinct nonces, 64 in flight (closed loop: the next request is
+submitted when one completes), payloads resident in HBM.  `value` is payload GB/s of the whole job.
+
+--backend engine (default) is the product path: the persistent kernel fed by the host-mapped ring.
+  The timed region is  [sync | aes_engine_start, K steps, aes_engine_stop | sync]: it contains the
+  one kernel launch the engine ever makes.
+--backend launch runs the same worker code through ordinary launches (aes_ctr_launch_batch, 64
+  requests per launch: the paper's own "stream + event" mechanism).  This is the form ncu can
+  replay, so the committed profiles are made with it; a persistent kernel that waits for host
+  submissions would deadlock under a serialising profiler.
+
+The JSON line also carries: roofline (binding unit = the shared-memory lookup crossbar, see
+DESIGN.md section 6; HBM fraction beside it), e2e (payloads in pinned HOST memory, read and written
+over PCIe inside the timed region), cpu_baseline (the oracle on the host cores, bounded sample),
+latency at 4 KiB (p50/p99 submit -> completion observed), clocks sampled during the timed region.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2607_02630_b200 import workloads  # noqa: E402
+
+MIB = 1 << 20
+METRIC = "aes_ctr_payload_throughput"
+UNIT = "GB/s"
+
+# shared-memory lookups per 16-byte block in the CUDA path: per block
+# 1 (round 1) + 4 (round 2) + 16 * (Nr - 2) ; plus 27 per 8 blocks for the per-row constants
+LOOKUPS = {128: 1 + 4 + 16 * 8 + 27 / 8.0, 256: 1 + 4 + 16 * 12 + 27 / 8.0}
+SMEM_BYTES_PER_CLK_PER_SM = 128.0  # 32 banks x 4 B (guides/B300_MICROARCH.md "smem crossbar BW")
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), float(d.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+# --------------------------------------------------------------------------------------------
+# clocks sampled DURING the timed region (NVML; the timed calls release the GIL)
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
+
+    def __init__(self, index: int):
+        self.samples, self.power, self.reasons = [], [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._th = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:  # noqa: BLE001
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:  # noqa: BLE001
+                pass
+            time.sleep(0.002)
+
+    def __enter__(self):
+        if self.nv:
+            self._th = threading.Thread(target=self._run, daemon=True)
+            self._th.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._th:
+            self._th.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# --------------------------------------------------------------------------------------------
+# workload set-up
+# --------------------------------------------------------------------------------------------
+def make_workload(name: str):
+    if name == "c2":
+        return workloads.config2(), 128
+    if name == "c3":
+        return workloads.config3(), 256
+    raise SystemExit("unknown workload %s" % name)
+
+
+def fill_payloads(w, dst_view_of):
+    """Writes the seeded payload of every request through dst_view_of(i) -> writable uint8 ndarray."""
+    for i in range(w.n):
+        dst_view_of(i)[:] = w.payload(i)
+
+
+def percentile(a, q):
+    return float(np.percentile(a, q)) if len(a) else None
+
+
+# --------------------------------------------------------------------------------------------
+# reference arm: the oracle on the host cores
+# --------------------------------------------------------------------------------------------
+def oracle_throughput(w, keybits, n_req, cores):
+    """Runs the oracle, as it stands, over the first n_req requests of w on `cores` threads.
+    Returns (GB/s, seconds)."""
+    import concurrent.futures as cf
+
+    from oracle import oracle as o
+
+    n_req = min(n_req, w.n)
+    size = int(w.length[0])
+    src = np.empty((n_req, size), dtype=np.uint8)
+    dst = np.empty_like(src)
+    for i in range(n_req):
+        src[i] = w.payload(i)
+    o.lib()
+
+    def one(i):
+        o.ctr_into(w.key_of(i), w.icb_of(i), src[i].ctypes.data, dst[i].ctypes.data, size)
+
+    t0 = time.perf_counter()
+    with cf.ThreadPoolExecutor(cores) as ex:
+        list(ex.map(one, range(n_req)))
+    dt = time.perf_counter() - t0
+    return n_req * size / dt / 1e9, dt
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w, keybits = make_workload(args.workload)
+    cores = len(os.sched_getaffinity(0))
+    per_step = max(cores, 16)  # requests per step: a bounded sample of the workload
+    for _ in range(args.warmup):
+        oracle_throughput(w, keybits, min(per_step, cores), cores)
+    t_total, b_total = 0.0, 0
+    for _ in range(args.steps):
+        gbs, dt = oracle_throughput(w, keybits, per_step, cores)
+        t_total += dt
+        b_total += per_step * int(w.length[0])
+    value = b_total / t_total / 1e9
+    sample = "%d of the %d requests of %s per step (%d MiB), %d threads" % (
+        per_step, w.n, w.name, per_step * int(w.length[0]) // MIB, cores)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": w.name, "sample": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+    return 0
+
+
+# --------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--backend", default="engine", choices=["engine", "launch"])
+    ap.add_argument("--workload", default="c2", choices=["c2", "c3"])
+    ap.add_argument("--chunk-rows", type=int, default=0)
+    ap.add_argument("--no-extras", action="store_true", help="skip e2e / latency / cpu_baseline / kernel-only legs")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.warmup < 3:
+        args.warmup = 3
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2607_02630_b200.binding as B
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    hbm_peak, sm_max_mhz, peak_kind = _peaks()
+    w, keybits = make_workload(args.workload)
+    size = int(w.length[0])
+    n = w.n
+
+    # ---- device-resident payloads (2 x n x size bytes: far larger than the 126 MB L2) ----
+    src = torch.empty(n * size, dtype=torch.uint8, device=dev)
+    dst = torch.empty(n * size, dtype=torch.uint8, device=dev)
+    stage = torch.empty(size, dtype=torch.uint8).pin_memory()
+    for i in range(n):
+        stage.numpy()[:] = w.payload(i)  # every rank uses the same seeded batch (weak scaling)
+        src[i * size:(i + 1) * size].copy_(stage)
+        torch.cuda.current_stream().synchronize()
+    dst.zero_()
+    torch.cuda.synchronize()
+    srcs = [src.data_ptr() + i * size for i in range(n)]
+    dsts = [dst.data_ptr() + i * size for i in range(n)]
+    lens = [size] * n
+    ctx = B.aes_ctx_create(w.key_of(0))
+    side = torch.cuda.Stream(device=dev)
+    launches0 = B.aes_engine_info()["kernel_launches"]
+
+    def step_engine():
+        r = B.aes_loop_run(w.icb, srcs, dsts, lens, window=w.in_flight, ctx=ctx, want_latency=False)
+        assert r["requests"] == n
+
+    LB = w.in_flight  # requests per ordinary launch in the launch backend
+
+    def step_launch(stream_ptr, events=None):
+        for b0 in range(0, n, LB):
+            b1 = min(n, b0 + LB)
+            if events is not None:
+                e0 = torch.cuda.Event(enable_timing=True)
+                e0.record()
+            B.aes_ctr_launch_batch([ctx] * (b1 - b0), w.icb[b0:b1], srcs[b0:b1], dsts[b0:b1], lens[b0:b1],
+                                   device=local_rank, cuda_stream=stream_ptr, chunk_rows=args.chunk_rows)
+            if events is not None:
+                e1 = torch.cuda.Event(enable_timing=True)
+                e1.record()
+                events.append((e0, e1, (b1 - b0) * size))
+
+    # ---- warm-up ----
+    if args.backend == "engine":
+        B.aes_engine_start(local_rank, chunk_rows=args.chunk_rows, idle_exit_ms=30000)
+        for _ in range(args.warmup):
+            step_engine()
+        B.aes_engine_stop()
+    else:
+        for _ in range(args.warmup):
+            step_launch(torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    barrier()
+
+    # ---- timed region: exactly K steps ----
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kernel_events = []
+    launches_before = B.aes_engine_info()["kernel_launches"]
+    with ClockSampler(local_rank) as clocks:
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        if args.backend == "engine":
+            ev0.record(side)
+            B.aes_engine_start(local_rank, chunk_rows=args.chunk_rows, idle_exit_ms=30000)
+            for _ in range(args.steps):
+                step_engine()
+            B.aes_engine_stop()
+            ev1.record(side)
+        else:
+            ev0.record()
+            for _ in range(args.steps):
+                step_launch(torch.cuda.current_stream().cuda_stream, kernel_events)
+            ev1.record()
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+    barrier()
+    gpu_launches = B.aes_engine_info()["kernel_launches"] - launches_before
+    ms_dev = ev0.elapsed_time(ev1)
+    ms_host = 1e3 * (t1 - t0)
+    tmax = torch.tensor([ms_dev], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_total = float(tmax.item())
+    bytes_per_step_all = n * size * world
+    value = bytes_per_step_all * args.steps / (ms_total * 1e-3) / 1e9
+    clk = clocks.summary()
+
+    # ---- parity spot check of what the timed region wrote (rank 0; oracle is test infrastructure) ----
+    verified = None
+    if rank == 0:
+        from oracle import oracle as o
+
+        ok = True
+        for i in (0, n // 2, n - 1):
+            got = dst[i * size:i * size + 8192].cpu().numpy().tobytes()
+            ok &= got == o.ctr(w.key_of(i), w.icb_of(i), w.payload(i)[:8192])
+            off = size - 4096
+            got = dst[i * size + off:(i + 1) * size].cpu().numpy().tobytes()
+            ok &= got == o.ctr(w.key_of(i), w.icb_of(i), w.payload(i)[off:], off // 16)
+        verified = bool(ok)
+
+    # ---- roofline of the dominant kernel (aesoff_engine_kernel) ----
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    sm_mhz = clk["sm_mhz"] or sm_max_mhz
+    lds_peak = SMEM_BYTES_PER_CLK_PER_SM * sm_count * sm_mhz * 1e6 / 1e9      # GB/s of lookup bytes
+    lds_per_payload_byte = LOOKUPS[keybits] * 4.0 / 16.0
+    if args.backend == "engine":
+        kern_payload_gbs = n * size * args.steps / (ms_dev * 1e-3) / 1e9
+        how = ("persistent kernel: one launch spans the timed region; achieved = algorithmic lookup bytes of the "
+               "K steps / CUDA-event time of the region (events on a side stream)")
+        kernel_ms = ms_dev
+    else:
+        per = [(e0.elapsed_time(e1), nb) for e0, e1, nb in kernel_events]
+        kernel_ms = float(np.mean([p[0] for p in per]))
+        kern_payload_gbs = float(np.mean([p[1] for p in per])) / (kernel_ms * 1e-3) / 1e9
+        how = "ordinary launches of %d requests; mean CUDA-event time per launch on the launching stream" % LB
+    roofline = {
+        "bound": "alu", "unit_detail": "shared-memory lookup crossbar (LSU), 4-byte lookups",
+        "kernel": "aesoff_engine_kernel",
+        "achieved": kern_payload_gbs * lds_per_payload_byte, "peak": lds_peak, "unit": "GB/s",
+        "frac": kern_payload_gbs * lds_per_payload_byte / lds_peak,
+        "peak_how": "128 B/clk/SM x %d SMs x %.0f MHz (SM clock sampled in the run)" % (sm_count, sm_mhz),
+        "lookups_per_block": LOOKUPS[keybits], "payload_gbs": kern_payload_gbs,
+        "hbm": {"achieved": 2 * kern_payload_gbs, "peak": hbm_peak, "unit": "GB/s",
+                "frac": 2 * kern_payload_gbs / hbm_peak, "peak_kind": peak_kind},
+        "traffic": None, "avg_launch_ms": kernel_ms, "how": how,
+    }
+
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "u8", "data": "synthetic",
+        "config": {"workload": w.name, "backend": args.backend, "keybits": keybits, "request_bytes": size,
+                   "requests_per_step": n, "in_flight": w.in_flight, "payload": "device-resident (HBM)",
+                   "l2": "inputs larger than L2 (%.1f GiB src + same dst per step)" % (n * size / 2**30),
+                   "seed": workloads.SEED_BASE + w.config_index},
+        "gpu_launches": int(gpu_launches), "ms_host": ms_host, "verified_vs_oracle": verified,
+        "clocks": clk, "roofline": roofline,
+    }
+
+    if not args.no_extras and rank == 0 and world == 1:
+        out.update(extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, size, n, step_launch,
+                          lds_per_payload_byte, lds_peak, hbm_peak))
+    elif rank == 0:
+        out["e2e"] = None
+    if rank == 0:
+        print(json.dumps(out))
+    B.aes_ctx_destroy(ctx)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, size, n, step_launch,
+           lds_per_payload_byte, lds_peak, hbm_peak):
+    res = {}
+    # ---- kernel-only leg: the worker code through ordinary launches, CUDA events per launch ----
+    if args.backend == "engine":
+        evs = []
+        step_launch(torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+        for _ in range(3):
+            step_launch(torch.cuda.current_stream().cuda_stream, evs)
+        torch.cuda.synchronize()
+        ms = float(np.mean([a.elapsed_time(b) for a, b, _ in evs]))
+        gbs = float(np.mean([nb for _, _, nb in evs])) / (ms * 1e-3) / 1e9
+        res["kernel_only"] = {"backend": "launch", "requests_per_launch": w.in_flight, "avg_launch_ms": ms,
+                              "payload_gbs": gbs, "lds_frac": gbs * lds_per_payload_byte / lds_peak,
+                              "hbm_frac": 2 * gbs / hbm_peak, "launches_timed": len(evs)}
+
+    # ---- e2e: payloads in pinned HOST memory, read and written by the kernel over PCIe ----
+    n_e2e = min(n, 256)
+    hs = B.aes_host_alloc(n_e2e * size)
+    hd = B.aes_host_alloc(n_e2e * size)
+    hsv, hdv = B.host_view(hs, n_e2e * size), B.host_view(hd, n_e2e * size)
+    for i in range(n_e2e):
+        hsv[i * size:(i + 1) * size] = w.payload(i)
+    hdv[:] = 0
+    hsrcs = [hs + i * size for i in range(n_e2e)]
+    hdsts = [hd + i * size for i in range(n_e2e)]
+    B.aes_engine_start(local_rank, chunk_rows=args.chunk_rows, idle_exit_ms=30000)
+    B.aes_loop_run(w.icb[:n_e2e], hsrcs, hdsts, lens[:n_e2e], window=w.in_flight, ctx=ctx, want_latency=False)
+    reps = 4
+    t0 = time.perf_counter()
+    r = B.aes_loop_run(w.icb[:n_e2e], hsrcs, hdsts, lens[:n_e2e], window=w.in_flight, ctx=ctx, repeat=reps,
+                       want_latency=False)
+    t1 = time.perf_counter()
+    from oracle import oracle as o
+
+    ok = hdv[:4096].tobytes() == o.ctr(w.key_of(0), w.icb_of(0), w.payload(0)[:4096])
+    e2e_gbs = r["bytes"] / (t1 - t0) / 1e9
+    res["e2e"] = {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": n_e2e * size, "d2h_bytes_per_step": n_e2e * size,
+                  "how": "aes_ctr_submit with src/dst in pinned host memory (aes_host_alloc): the kernel reads the "
+                         "payload and writes the result over PCIe inside the timed region; %d requests x %d B, %d in "
+                         "flight, %d repeats" % (n_e2e, size, w.in_flight, reps),
+                  "verified_vs_oracle": bool(ok)}
+
+    # ---- latency at 4 KiB (the metric's second half), device-resident, 1 and 256 in flight ----
+    lat = {}
+    nl = 10000
+    small = 4096
+    pool = 512
+    lsrc = torch.empty(pool * small, dtype=torch.uint8, device=dev)  # no kernel: contents are irrelevant to timing
+    ldst = torch.empty(pool * small, dtype=torch.uint8, device=dev)
+    wl = workloads.fixed_size(small, nl, 1)
+    ls = [lsrc.data_ptr() + (i % pool) * small for i in range(nl)]
+    ld = [ldst.data_ptr() + (i % pool) * small for i in range(nl)]
+    for depth in (1, 256):
+        r = B.aes_loop_run(wl.icb, ls, ld, [small] * nl, window=depth, ctx=ctx)
+        a = r["lat_ns"][nl // 20:] / 1e3
+        lat["inflight_%d" % depth] = {"p50_us": percentile(a, 50), "p99_us": percentile(a, 99),
+                                      "mean_us": float(a.mean()), "req_per_s": nl / (r["elapsed_ns"] * 1e-9)}
+    res["latency_4KiB"] = lat
+    B.aes_engine_stop()
+    # freeing pinned memory synchronises the device, so only after the engine has stopped
+    del hsv, hdv
+    B.aes_host_free(hs)
+    B.aes_host_free(hd)
+
+    # ---- cpu_baseline: the oracle, as it stands, on the host cores, bounded sample ----
+    cores = len(os.sched_getaffinity(0))
+    n_cpu = min(n, 16 * cores)
+    gbs, dt = oracle_throughput(w, keybits, n_cpu, cores)
+    res["cpu_baseline"] = {"value": gbs, "unit": UNIT, "cores": cores, "kind": "oracle",
+                           "sample": "first %d of %d requests of %s (%d MiB), one thread per core, %.1f s" % (
+                               n_cpu, n, w.name, n_cpu * size // MIB, dt)}
+    return res
+
+
+if __name__ == "__main__":
+    sys.exit(main())

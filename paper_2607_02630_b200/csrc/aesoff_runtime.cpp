@@ -209,6 +209,10 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
     if (major != 10) return fail(AES_E_CUDA); /* sm_100a code only */
 
+    /* ring, mailbox and queues survive a stop/start cycle with the same geometry (a restart then costs
+     * one launch, not a dozen allocations) */
+    const bool reuse = e.hring && e.device == device && e.R == o.ring_slots;
+    if (!reuse) free_engine_memory(e);
     e.device = device;
     e.sm_count = sms;
     e.n_ctas = o.n_ctas ? (int)o.n_ctas : sms;
@@ -219,6 +223,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     e.first_seq = e.next_seq.load();
 
     bool ok = true;
+    if (!reuse) {
     ok = ok && cudaStreamCreateWithFlags(&e.stream, cudaStreamNonBlocking) == cudaSuccess;
     const unsigned hflags = cudaHostAllocMapped | cudaHostAllocPortable;
     ok = ok && cudaHostAlloc((void **)&e.hring, (size_t)e.R * sizeof(aesoff_host_slot_t), hflags) == cudaSuccess;
@@ -236,11 +241,13 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     }
     memset(e.hring, 0, (size_t)e.R * sizeof(aesoff_host_slot_t));
     memset(e.hmail, 0, (size_t)e.R * 8);
-    memset(e.hctl, 0, AESOFF_CTL_WORDS * 4);
-    ok = ok && cudaMemset(e.counters, 0, AESOFF_CNT_WORDS * 8) == cudaSuccess;
     ok = ok && cudaMemset(e.dev_done_seq, 0, (size_t)e.R * 8) == cudaSuccess;
-    ok = ok && cudaMemset(e.dq_done, 0, (size_t)e.R * 4) == cudaSuccess;
     ok = ok && cudaMemcpy(e.dT0, aesoff_T0_table(), 256 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+    }
+    /* sequence numbers never restart, so stale slot/mailbox values (< first_seq) can never match */
+    memset(e.hctl, 0, AESOFF_CTL_WORDS * 4);
+    ok = ok && cudaMemsetAsync(e.counters, 0, AESOFF_CNT_WORDS * 8, e.stream) == cudaSuccess;
+    ok = ok && cudaMemsetAsync(e.dq_done, 0, (size_t)e.R * 4, e.stream) == cudaSuccess;
     if (!ok) {
         free_engine_memory(e);
         return fail(AES_E_CUDA);
@@ -306,7 +313,7 @@ extern "C" int aes_engine_stop(void)
     }
     __atomic_store_n(&e.hctl[AESOFF_CTL_STOP], 1u, __ATOMIC_RELEASE);
     if (cudaStreamSynchronize(e.stream) != cudaSuccess) rc = AES_E_CUDA;
-    free_engine_memory(e);
+    if (rc != AES_OK) free_engine_memory(e); /* otherwise kept for the next start */
     e.running.store(0, std::memory_order_release);
     if (rc != AES_OK) return fail(rc);
     return AES_OK;
