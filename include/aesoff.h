@@ -59,10 +59,12 @@ typedef uint64_t       aes_handle_t;  /* submission sequence number, from 1; 0 =
 
 /* ---- engine life cycle (step a0 of the path) -------------------------------
  * The engine is: a pinned, host-mapped descriptor ring; ONE persistent sm_100a
- * kernel (a dispatcher warp that polls the ring over PCIe plus worker groups
- * that hold the AES tables in shared memory); and a host-mapped completion
+ * kernel (a dispatcher warp that polls the ring over PCIe, and per SM one
+ * service warp plus 16 worker warps around the AES tables in shared memory);
+ * and a host-mapped completion
  * mailbox.  A request therefore never pays a kernel launch (the paper's 4 KiB
  * point is "launch-bound").                                       */
+#define AES_FINE_ROWS_OFF 0xffffffffu
 typedef struct aes_engine_opts {
     uint32_t ring_slots;      /* descriptor ring depth = max requests in flight; power of
                                  two in [64, 4096]; 0 = default 2048                      */
@@ -71,7 +73,12 @@ typedef struct aes_engine_opts {
     uint32_t n_ctas;          /* persistent CTAs; 0 = one per SM                          */
     uint32_t idle_exit_ms;    /* the kernel exits by itself (engine becomes STOPPED) after
                                  this long with no request; 0 = never                     */
-    uint32_t reserved[4];     /* must be 0                                                */
+    uint32_t fine_rows;       /* latency mode: a request of at most this many 4 KiB rows is
+                                 cut into 1/8-row units (32 blocks per warp instead of 256)
+                                 when the GPU has idle CTAs, so that it spreads over many
+                                 warps; requests up to 16 rows always are.  0 = default 512,
+                                 AES_FINE_ROWS_OFF = never                                 */
+    uint32_t reserved[3];     /* must be 0                                                */
 } aes_engine_opts_t;
 
 /* Starts the engine on CUDA device `device`.  opts == NULL means all defaults.
@@ -92,7 +99,7 @@ typedef struct aes_engine_info {
     int32_t  sm_count;
     int32_t  n_ctas;
     int32_t  threads_per_cta;
-    int32_t  groups_per_cta;     /* worker groups (128 threads each) per CTA         */
+    int32_t  worker_warps_per_cta; /* warps that run the cipher (the rest: service, dispatcher) */
     uint32_t ring_slots;
     uint32_t chunk_rows;
     uint32_t smem_bytes_per_cta;

@@ -20,6 +20,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libaesoff.so")
 
 AES_OK = 0
+AES_FINE_ROWS_OFF = 0xFFFFFFFF
 AES_E_INVAL = -1
 AES_E_KEYBITS = -2
 AES_E_ALIGN = -3
@@ -40,12 +41,12 @@ class AesOffError(RuntimeError):
 
 class aes_engine_opts_t(ctypes.Structure):
     _fields_ = [("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32), ("n_ctas", ctypes.c_uint32),
-                ("idle_exit_ms", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 4)]
+                ("idle_exit_ms", ctypes.c_uint32), ("fine_rows", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 3)]
 
 
 class aes_engine_info_t(ctypes.Structure):
     _fields_ = [("running", ctypes.c_int32), ("device", ctypes.c_int32), ("sm_count", ctypes.c_int32),
-                ("n_ctas", ctypes.c_int32), ("threads_per_cta", ctypes.c_int32), ("groups_per_cta", ctypes.c_int32),
+                ("n_ctas", ctypes.c_int32), ("threads_per_cta", ctypes.c_int32), ("worker_warps_per_cta", ctypes.c_int32),
                 ("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32),
                 ("smem_bytes_per_cta", ctypes.c_uint32), ("reserved0", ctypes.c_uint32),
                 ("submitted", ctypes.c_uint64), ("completed", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64)]
@@ -115,8 +116,8 @@ def _check(rc: int, where: str) -> None:
 
 # ---- engine ---------------------------------------------------------------------------------
 def aes_engine_start(device: int = 0, ring_slots: int = 0, chunk_rows: int = 0, n_ctas: int = 0,
-                     idle_exit_ms: int = 0) -> None:
-    o = aes_engine_opts_t(ring_slots, chunk_rows, n_ctas, idle_exit_ms)
+                     idle_exit_ms: int = 0, fine_rows: int = 0) -> None:
+    o = aes_engine_opts_t(ring_slots, chunk_rows, n_ctas, idle_exit_ms, fine_rows)
     _check(_lib.aes_engine_start(device, ctypes.byref(o)), "aes_engine_start")
 
 

@@ -1,83 +1,75 @@
 /*
- * aesoff_kernels.cu -- the sm_100a device side of the AES-CTR offload engine.
+ * aesoff_kernels.cu -- the sm_100a engine kernel of the AES-CTR offload engine.
  *
  * One kernel, `aesoff_engine_kernel`, in two modes:
- *   PERSISTENT  launched once by aes_engine_start(); a dispatcher warp polls the host-mapped
- *               descriptor ring over PCIe and hands chunks to worker groups; lives until
- *               aes_engine_stop().  This is what replaces the paper's "own CUDA stream, polled
- *               by cudaEventQuery" path that is launch-bound at 4 KiB.
- *   DRAIN       the same worker code over a queue the host filled before an ordinary launch
+ *   PERSISTENT  launched once by aes_engine_start(); lives until aes_engine_stop().  This is what
+ *               replaces the paper's "own CUDA stream, polled by cudaEventQuery" path that is
+ *               launch-bound at 4 KiB.
+ *   DRAIN       the same code over a queue the host filled before an ordinary launch
  *               (aes_ctr_launch_batch); exits when the queue is empty.  This is the paper's own
  *               mechanism and the form ncu can replay.
  *
- * The arithmetic (steps a4-a6 of SURVEY.md section 8(a)):
- *   FIPS-197 Cipher() with the SubBytes/ShiftRows/MixColumns of a round folded into four
- *   256-entry word tables (the classical "T-table" form of sec. 5.1: column j of a round's output
- *   is T0[s0,j] ^ T1[s1,j+1] ^ T2[s2,j+2] ^ T3[s3,j+3] ^ roundkey), SP 800-38A sec. 6.5 CTR around it.
- *
- * B200 specifics:
- *   - The binding unit is the shared-memory crossbar: 32 four-byte lookups per clock per SM.  Each of
- *     the four tables is therefore replicated once per bank (lane l only ever reads bank l), which
- *     makes every LDS conflict-free by construction: 4 x 256 x 32 x 4 B = 128 KiB per SM.
- *   - Entries sit at a 256-byte stride (two tables interleaved per 64 KiB region) so that one PRMT
- *     builds the whole lookup address  (byte_k(x) << 8) | lane*4 | region_base.
- *   - CTR structure: a warp works on one "row" = the 256 counter values that share the upper 120
- *     counter bits.  Everything of rounds 1 and 2 that depends only on those bits is computed once
- *     per row; per block round 1 is ONE lookup and round 2 FOUR (133 instead of 160 lookups per
- *     AES-128 block, 197 instead of 224 for AES-256).
- *   - Payload is read/written with 128-bit L2-only accesses (ld.global.cg / st.global.cg): a
- *     persistent kernel never gets its L1 invalidated, so a recycled request buffer must not hit L1.
+ * Roles inside a CTA (one CTA per SM):
+ *   warps 0..15   WORKERS.  A worker claims one *unit* (a 4 KiB row of one request, or 1/8 of a row
+ *                 in latency mode) from the CTA's slot queue in shared memory and runs the cipher
+ *                 over it (aesoff_cipher.cuh).  Workers never wait on global memory except for the
+ *                 payload itself: no barriers, no ticket round trips.
+ *   warp 16       SERVICE.  Keeps the CTA's AESOFF_SLOTS slots filled: reserves chunk tickets from
+ *                 the device-wide ticket counter, waits until the dispatcher has published them,
+ *                 copies the 320-byte descriptor (round keys included) into the slot and opens it
+ *                 for claiming -- all while the workers are busy with earlier slots.
+ *   warp 17       DISPATCHER (CTA 0, persistent mode only).  Polls the host-mapped descriptor ring
+ *                 over PCIe, copies request bodies into the device queue and cuts each request into
+ *                 chunk tickets (step a3).
+ * Completion (step a7): the worker that finishes the last unit of a slot counts the request's chunks
+ * down in global memory; the last chunk's finisher fences at system scope and writes the request's
+ * sequence number into the host-mapped mailbox.
  */
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "aesoff_cipher.cuh"
 #include "aesoff_shared.h"
+
+using namespace aesoff;
 
 namespace {
 
 /* ------------------------------------------------------------------------------------------ */
-/* shared-memory table layout                                                                  */
+/* per-CTA control block in shared memory                                                      */
 /* ------------------------------------------------------------------------------------------ */
-constexpr int OFF_T0 = 0;
-constexpr int OFF_T1 = 128;
-constexpr int OFF_T2 = 65536;
-constexpr int OFF_T3 = 65536 + 128;
-constexpr uint32_t TABLE_BYTES = 131072;
+struct __align__(16) Slot {
+    aesoff_dev_desc_t desc; /* 320 B: descriptor of the request, round keys included            */
+    uint32_t unit0_row;     /* first row of this chunk                                          */
+    uint32_t ring_slot;     /* index of the request in dq / mailbox                             */
+    uint32_t n_units;
+    uint32_t fine;          /* 1: a unit is one k-iteration (32 blocks) of a row, else a row    */
+};                          /* 336 B */
 
-struct __align__(16) GroupCtl {
-    aesoff_dev_desc_t desc;      /* 320 B: descriptor of the request this group last worked on */
-    unsigned long long entry;    /* ticket entry handed from the group leader to the group      */
-    unsigned long long pad[7];
-};                               /* 384 B */
-constexpr uint32_t CTRL_BYTES = sizeof(GroupCtl) * AESOFF_GROUPS_PER_CTA;
-constexpr unsigned long long ENTRY_EXIT = ~0ull;
+struct __align__(16) CtaCtl {
+    Slot slot[AESOFF_SLOTS];
+    /* claim[s] = n_units << 16 | next unit.  Written whole by the service warp when it opens the
+     * slot (after the descriptor), incremented by claiming workers: one atomic snapshot tells a
+     * worker both the unit it got and whether that unit exists.                                 */
+    uint32_t claim[AESOFF_SLOTS];
+    uint32_t done[AESOFF_SLOTS];  /* units finished                                              */
+    uint32_t stamp[AESOFF_SLOTS]; /* fill order, so that workers take the oldest open slot first */
+    uint32_t busy[AESOFF_SLOTS];  /* 0 free, 1 filled and not yet completed                      */
+    uint32_t exit_flag;
+    uint32_t pad[3];
+};
+constexpr uint32_t CTRL_BYTES = sizeof(CtaCtl);
+constexpr uint32_t CLAIM_EXIT = 0xffffffffu;
 
-template <int OFF>
-__device__ __forceinline__ uint32_t lds_off(uint32_t a)
+__device__ __forceinline__ uint32_t lds_volatile(const uint32_t *p)
 {
     uint32_t v;
-    asm("ld.shared.u32 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF));
+    asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(v) : "r"((uint32_t)__cvta_generic_to_shared(p)) : "memory");
     return v;
 }
-__device__ __forceinline__ void sts(uint32_t a, uint32_t v)
+__device__ __forceinline__ void sts_volatile(uint32_t *p, uint32_t v)
 {
-    asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(v) : "memory");
-}
-/* (byte K of x) << 8 | ybase, where ybase = region_base | lane*4 and region_base % 65536 == 0 */
-template <int K>
-__device__ __forceinline__ uint32_t taddr(uint32_t x, uint32_t ybase)
-{
-    return __byte_perm(x, ybase, 0x7604 | (K << 4));
-}
-#define TL(T, K, x) lds_off<OFF_T##T>(taddr<K>((x), ybase))
-
-__device__ __forceinline__ uint32_t bswap32(uint32_t x) { return __byte_perm(x, 0, 0x0123); }
-__device__ __forceinline__ uint32_t rotl32(uint32_t x, int n) { return __funnelshift_l(x, x, n); }
-__device__ __forceinline__ uint32_t bitsel(uint32_t a, uint32_t b, uint32_t m) { return (a & m) | (b & ~m); }
-
-__device__ __forceinline__ void group_sync(int group)
-{
-    asm volatile("bar.sync %0, %1;" ::"r"(group + 1), "n"(AESOFF_GROUP_THREADS) : "memory");
+    asm volatile("st.volatile.shared.u32 [%0], %1;" ::"r"((uint32_t)__cvta_generic_to_shared(p)), "r"(v) : "memory");
 }
 __device__ __forceinline__ unsigned long long ld_acquire_gpu(const unsigned long long *p)
 {
@@ -117,217 +109,205 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
     return t;
 }
 
-/* at most one block per request takes this path, so it is kept out of line */
-__device__ __noinline__ void store_partial(const uint8_t *src, uint8_t *dst, uint32_t o0, uint32_t o1, uint32_t o2,
-                                           uint32_t o3, uint32_t u)
+/* ------------------------------------------------------------------------------------------ */
+/* worker warp (steps a4-a7)                                                                   */
+/* ------------------------------------------------------------------------------------------ */
+/* Takes a unit of the oldest open slot.  Returns slot << 16 | unit, or CLAIM_EXIT.             */
+__device__ __forceinline__ uint32_t claim_unit(CtaCtl *c, uint32_t lane)
 {
-#pragma unroll 1
-    for (uint32_t i = 0; i < u; ++i) {
-        const uint32_t w = (i < 8) ? (i < 4 ? o0 : o1) : (i < 12 ? o2 : o3);
-        const uint8_t ks = (uint8_t)(w >> (8u * (i & 3u)));
-        const uint8_t pt = __ldcg(src + i);
-        __stcg(dst + i, (uint8_t)(pt ^ ks));
+    for (;;) {
+        uint32_t w = 0, st = 0;
+        if (lane < AESOFF_SLOTS) {
+            w = lds_volatile(&c->claim[lane]);
+            st = lds_volatile(&c->stamp[lane]);
+        }
+        const uint32_t avail = __ballot_sync(0xffffffffu, (w & 0xffffu) < (w >> 16));
+        if (avail) {
+            /* oldest first; live stamps lie within AESOFF_SLOTS of each other, so the signed
+             * distance to any live one orders them even when the counter wraps                  */
+            const uint32_t ref = __shfl_sync(0xffffffffu, st, __ffs(avail) - 1);
+            uint32_t key = 0xffffffffu;
+            if ((avail >> lane) & 1u) key = ((st - ref + 0x1000u) << 5) | lane;
+            const uint32_t s = __reduce_min_sync(0xffffffffu, key) & 31u;
+            uint32_t v = 0;
+            if (lane == 0) v = atomicAdd(&c->claim[s], 1u);
+            if (lane == 0) __threadfence_block(); /* acquire side of the service warp's slot publication */
+            v = __shfl_sync(0xffffffffu, v, 0);
+            __syncwarp();
+            if ((v & 0xffffu) < (v >> 16)) return (s << 16) | (v & 0xffffu);
+            continue;
+        }
+        if (lds_volatile(&c->exit_flag)) return CLAIM_EXIT;
+        __nanosleep(40);
+    }
+}
+
+/* The slot's chunk is finished: count the request's chunks down; the last one signals the host. */
+__device__ __forceinline__ void complete_chunk(const aesoff_params_t &P, CtaCtl *c, uint32_t s)
+{
+    const Slot *sl = &c->slot[s];
+    const uint32_t ring = sl->ring_slot, nchunks = sl->desc.nchunks;
+    const unsigned long long seq = sl->desc.seq;
+    /* the other workers' stores to dst happen-before their done-count increments (fence.cta +
+     * shared-memory atomic), which this thread has observed: this fence is cumulative over them */
+    __threadfence();
+    bool last = true;
+    if (nchunks > 1) {
+        const uint32_t d = atomicAdd(P.dq_done + ring, 1u);
+        last = (d + 1 == nchunks);
+        if (last) P.dq_done[ring] = 0;
+    }
+    if (last) {
+        __threadfence_system();
+        if (P.hmail) P.hmail[ring] = seq;
+        *reinterpret_cast<volatile uint64_t *>(P.dev_done_seq + ring) = seq;
+    }
+    sts_volatile(&c->busy[s], 0u); /* the service warp may refill the slot */
+}
+
+__device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase, uint32_t lane)
+{
+    for (;;) {
+        const uint32_t got = claim_unit(c, lane);
+        if (got == CLAIM_EXIT) break;
+        const uint32_t s = got >> 16, u = got & 0xffffu;
+        const Slot *sl = &c->slot[s];
+        const uint4 *rk4 = reinterpret_cast<const uint4 *>(sl->desc.rk);
+        const int nr = (int)sl->desc.nr;
+        const uint64_t len = sl->desc.len;
+        const uint8_t *src = reinterpret_cast<const uint8_t *>(sl->desc.src);
+        uint8_t *dst = reinterpret_cast<uint8_t *>(sl->desc.dst);
+        const CtrGeom g = ctr_geom(sl->desc.icb[0], sl->desc.icb[1], sl->desc.icb[2], sl->desc.icb[3]);
+        const uint32_t n_units = sl->n_units;
+        if (sl->fine) {
+            const uint64_t m = (uint64_t)sl->unit0_row + (u >> 3);
+            ctr_request_row<1>(ybase, rk4, nr, g, src, dst, len, m, lane, u & 7u, (u & 7u) + 1u);
+        } else {
+            const uint64_t m = (uint64_t)sl->unit0_row + u;
+            ctr_request_row<4>(ybase, rk4, nr, g, src, dst, len, m, lane);
+        }
+        __syncwarp();
+        if (lane == 0) {
+            __threadfence_block();
+            const uint32_t d = atomicAdd(&c->done[s], 1u);
+            if (d + 1 == n_units) complete_chunk(P, c, s);
+        }
+        __syncwarp();
     }
 }
 
 /* ------------------------------------------------------------------------------------------ */
-/* one row: the (up to) 256 blocks whose counter blocks share bytes 0..14                      */
+/* service warp: global ticket queue -> this CTA's slots, ahead of the workers  (a3)           */
 /* ------------------------------------------------------------------------------------------ */
-/* U0..U3   the counter block with its last byte zero, as four little-endian-loaded words
- * rk4      round keys in shared memory (uint4 per round)
- * src_row  address the block with last counter byte 0 would have (may lie before the payload)
- * lo_L     first valid value of the last counter byte in this row (non-zero only in row 0)
- * row_bytes  payload bytes from src_row to the end of the payload, capped at 4096
- * Lane l computes blocks L = l + 32k, k = 0..7, NB at a time.                                  */
-template <int NB>
-__device__ __forceinline__ void ctr_row(uint32_t ybase, const uint4 *rk4, int nr, uint32_t U0, uint32_t U1,
-                                        uint32_t U2, uint32_t U3, const uint8_t *src_row, uint8_t *dst_row,
-                                        uint32_t lo_L, uint32_t row_bytes, uint32_t lane)
-{
-    const uint4 k0 = rk4[0], k1 = rk4[1], k2 = rk4[2];
-    /* round 0 (AddRoundKey) on the row's common counter block */
-    const uint32_t s0 = U0 ^ k0.x, s1 = U1 ^ k0.y, s2 = U2 ^ k0.z, s3 = U3 ^ k0.w;
-    /* round 1: columns 1..3 do not see the last counter byte at all, column 0 sees it through T3 */
-    const uint32_t K1_0 = TL(0, 0, s0) ^ TL(1, 1, s1) ^ TL(2, 2, s2) ^ k1.x;
-    const uint32_t C1 = TL(0, 0, s1) ^ TL(1, 1, s2) ^ TL(2, 2, s3) ^ TL(3, 3, s0) ^ k1.y;
-    const uint32_t C2 = TL(0, 0, s2) ^ TL(1, 1, s3) ^ TL(2, 2, s0) ^ TL(3, 3, s1) ^ k1.z;
-    const uint32_t C3 = TL(0, 0, s3) ^ TL(1, 1, s0) ^ TL(2, 2, s1) ^ TL(3, 3, s2) ^ k1.w;
-    /* round 2: per column, the three lookups fed by the constant columns C1..C3 */
-    const uint32_t K2_0 = TL(1, 1, C1) ^ TL(2, 2, C2) ^ TL(3, 3, C3) ^ k2.x;
-    const uint32_t K2_1 = TL(0, 0, C1) ^ TL(1, 1, C2) ^ TL(2, 2, C3) ^ k2.y;
-    const uint32_t K2_2 = TL(0, 0, C2) ^ TL(1, 1, C3) ^ TL(3, 3, C1) ^ k2.z;
-    const uint32_t K2_3 = TL(0, 0, C3) ^ TL(2, 2, C1) ^ TL(3, 3, C2) ^ k2.w;
-    /* address of T3[state byte 15] for last counter byte 0; the byte itself is xored in per block */
-    const uint32_t a3 = taddr<3>(s3, ybase) ^ (lane << 8);
-
-#pragma unroll 1
-    for (uint32_t kb = 0; kb < 8; kb += NB) {
-        if (kb * 512u >= row_bytes) break;           /* warp-uniform: nothing left in this row  */
-        if ((kb + NB) * 32u <= lo_L) continue;       /* warp-uniform: still before the payload  */
-        uint4 p[NB];
-        uint32_t st[NB][4];
-        bool full[NB];
-#pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            const uint32_t L = lane + 32u * (kb + b), off = L * 16u;
-            full[b] = (L >= lo_L) && (off + 16u <= row_bytes);
-            p[b] = make_uint4(0, 0, 0, 0);
-            if (full[b]) p[b] = __ldcg(reinterpret_cast<const uint4 *>(src_row + off));
-        }
-        /* rounds 1 and 2: 1 + 4 lookups per block */
-#pragma unroll
-        for (int b = 0; b < NB; ++b) {
-            const uint32_t r1 = K1_0 ^ lds_off<OFF_T3>(a3 ^ ((kb + b) << 13));
-            st[b][0] = K2_0 ^ TL(0, 0, r1);
-            st[b][1] = K2_1 ^ TL(3, 3, r1);
-            st[b][2] = K2_2 ^ TL(2, 2, r1);
-            st[b][3] = K2_3 ^ TL(1, 1, r1);
-        }
-        /* rounds 3 .. Nr-1: 16 lookups per block per round */
-#pragma unroll 1
-        for (int r = 3; r < nr; ++r) {
-            const uint4 kk = rk4[r];
-#pragma unroll
-            for (int b = 0; b < NB; ++b) {
-                const uint32_t x0 = st[b][0], x1 = st[b][1], x2 = st[b][2], x3 = st[b][3];
-                st[b][0] = TL(0, 0, x0) ^ TL(1, 1, x1) ^ TL(2, 2, x2) ^ TL(3, 3, x3) ^ kk.x;
-                st[b][1] = TL(0, 0, x1) ^ TL(1, 1, x2) ^ TL(2, 2, x3) ^ TL(3, 3, x0) ^ kk.y;
-                st[b][2] = TL(0, 0, x2) ^ TL(1, 1, x3) ^ TL(2, 2, x0) ^ TL(3, 3, x1) ^ kk.z;
-                st[b][3] = TL(0, 0, x3) ^ TL(1, 1, x0) ^ TL(2, 2, x1) ^ TL(3, 3, x2) ^ kk.w;
-            }
-        }
-        /* final round: SubBytes + ShiftRows + AddRoundKey.  S[x] is read out of the T entries:
-         * T3 has it in byte 0, T0 in bytes 1 and 2, T1 in byte 3.                                */
-        {
-            const uint4 kk = rk4[nr];
-#pragma unroll
-            for (int b = 0; b < NB; ++b) {
-                const uint32_t x0 = st[b][0], x1 = st[b][1], x2 = st[b][2], x3 = st[b][3];
-                uint32_t o[4];
-                o[0] = bitsel(bitsel(TL(3, 0, x0), TL(0, 1, x1), 0x000000ffu),
-                              bitsel(TL(0, 2, x2), TL(1, 3, x3), 0x00ff0000u), 0x0000ffffu) ^ kk.x;
-                o[1] = bitsel(bitsel(TL(3, 0, x1), TL(0, 1, x2), 0x000000ffu),
-                              bitsel(TL(0, 2, x3), TL(1, 3, x0), 0x00ff0000u), 0x0000ffffu) ^ kk.y;
-                o[2] = bitsel(bitsel(TL(3, 0, x2), TL(0, 1, x3), 0x000000ffu),
-                              bitsel(TL(0, 2, x0), TL(1, 3, x1), 0x00ff0000u), 0x0000ffffu) ^ kk.z;
-                o[3] = bitsel(bitsel(TL(3, 0, x3), TL(0, 1, x0), 0x000000ffu),
-                              bitsel(TL(0, 2, x1), TL(1, 3, x2), 0x00ff0000u), 0x0000ffffu) ^ kk.w;
-                const uint32_t L = lane + 32u * (kb + b), off = L * 16u;
-                if (full[b]) {
-                    uint4 c;
-                    c.x = p[b].x ^ o[0];
-                    c.y = p[b].y ^ o[1];
-                    c.z = p[b].z ^ o[2];
-                    c.w = p[b].w ^ o[3];
-                    __stcg(reinterpret_cast<uint4 *>(dst_row + off), c);
-                } else if (L >= lo_L && off < row_bytes) {
-                    /* the request's final partial block: leading bytes of O_n (SP 800-38A 6.5) */
-                    store_partial(src_row + off, dst_row + off, o[0], o[1], o[2], o[3], row_bytes - off);
-                }
-            }
-        }
-    }
-}
-
-/* ------------------------------------------------------------------------------------------ */
-/* one chunk of a request, by one worker group (4 warps; warp w takes rows w, w+4, ...)        */
-/* ------------------------------------------------------------------------------------------ */
-__device__ __forceinline__ void process_chunk(const GroupCtl *g, uint32_t ybase, uint32_t chunk, uint32_t warp_in_group,
-                                              uint32_t lane)
-{
-    const uint4 *rk4 = reinterpret_cast<const uint4 *>(g->desc.rk);
-    const int nr = (int)g->desc.nr;
-    const uint64_t len = g->desc.len;
-    const uint8_t *src = reinterpret_cast<const uint8_t *>(g->desc.src);
-    uint8_t *dst = reinterpret_cast<uint8_t *>(g->desc.dst);
-    const uint32_t crows = g->desc.chunk_rows;
-    const uint64_t rows = g->desc.rows;
-    /* SP 800-38A B.1 standard incrementing function with m = 128: the counter block is a
-     * big-endian integer.  c0 = its last byte; rows are aligned on that byte being 0.        */
-    const uint32_t i0 = g->desc.icb[0], i1 = g->desc.icb[1], i2 = g->desc.icb[2], i3 = g->desc.icb[3];
-    const uint32_t c0 = i3 >> 24;
-    const uint64_t hi = ((uint64_t)bswap32(i0) << 32) | bswap32(i1);
-    const uint64_t lo_cleared = (((uint64_t)bswap32(i2) << 32) | bswap32(i3)) & ~0xffull;
-
-    const uint64_t row_begin = (uint64_t)chunk * crows;
-    uint64_t row_end = row_begin + crows;
-    if (row_end > rows) row_end = rows;
-    for (uint64_t m = row_begin + warp_in_group; m < row_end; m += AESOFF_GROUP_THREADS / 32) {
-        const uint64_t l2 = lo_cleared + (m << 8);
-        const uint64_t h2 = hi + (l2 < lo_cleared ? 1ull : 0ull);
-        const uint32_t U0 = bswap32((uint32_t)(h2 >> 32)), U1 = bswap32((uint32_t)h2);
-        const uint32_t U2 = bswap32((uint32_t)(l2 >> 32)), U3 = bswap32((uint32_t)l2);
-        const int64_t row_off = ((int64_t)(m << 8) - (int64_t)c0) * 16;
-        const int64_t avail = (int64_t)len - row_off;
-        const uint32_t row_bytes = avail >= (int64_t)AESOFF_ROW_BYTES ? AESOFF_ROW_BYTES : (uint32_t)avail;
-        const uint32_t lo_L = (m == 0) ? c0 : 0u;
-        ctr_row<4>(ybase, rk4, nr, U0, U1, U2, U3, src + row_off, dst + row_off, lo_L, row_bytes, lane);
-    }
-}
-
-/* ------------------------------------------------------------------------------------------ */
-/* worker group: claim a ticket, wait until it is published, process, count down (a3, a7)      */
-/* ------------------------------------------------------------------------------------------ */
-__device__ void worker_loop(const aesoff_params_t &P, GroupCtl *g, uint32_t ybase, int group, uint32_t gtid)
+/* Lane j < AESOFF_SLOTS owns slot j.  All lanes run in lock step; nothing here is on the
+ * workers' critical path as long as at least one slot is open.                                 */
+__device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
 {
     unsigned long long *g_ticket = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_TICKET);
-    unsigned long long *g_published = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_PUBLISHED);
-    unsigned long long *g_stop = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_STOP);
-    unsigned long long pub_seen = 0;
-    unsigned long long cached_seq = 0;
-    const uint32_t warp_in_group = gtid >> 5, lane = gtid & 31u;
+    const bool persistent = (P.mode == AESOFF_MODE_PERSISTENT);
+    const bool mine = lane < AESOFF_SLOTS;
+    unsigned long long *g_idle = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_IDLE);
+    bool have = false;          /* this lane holds a reserved ticket for its (free) slot */
+    unsigned long long t = 0;   /* that ticket */
+    uint32_t stamp_base = 0;
+    bool counted_idle = false;  /* this CTA is included in the device-wide idle-CTA count */
 
     for (;;) {
-        if (gtid == 0) {
-            unsigned long long e = ENTRY_EXIT;
-            const unsigned long long t = atomicAdd(g_ticket, 1ull);
-            if (P.mode == AESOFF_MODE_DRAIN) {
-                if (t < P.drain_total) e = __ldcg(P.tmap + (t & (P.TM - 1)));
-            } else {
-                bool stop = false;
-                while (pub_seen <= t) {
-                    pub_seen = ld_acquire_gpu(g_published);
-                    if (pub_seen > t) break;
-                    if (ld_acquire_gpu(g_stop) != 0) {
-                        stop = true;
-                        break;
-                    }
-                    __nanosleep(100);
+        const bool is_free = mine && lds_volatile(&c->busy[lane]) == 0u;
+        const uint32_t busy_mask = __ballot_sync(0xffffffffu, mine && !is_free);
+        const uint32_t have_mask = __ballot_sync(0xffffffffu, have);
+        uint32_t need = __ballot_sync(0xffffffffu, is_free && !have);
+        if (persistent && (busy_mask == 0u) != counted_idle) {
+            /* the dispatcher cuts requests fine only while a good part of the GPU has nothing to do */
+            counted_idle = !counted_idle;
+            if (lane == 0) atomicAdd(g_idle, counted_idle ? 1ull : ~0ull);
+        }
+
+        /* ticket counter and published count sit in one 16-byte word: one L2 read gives both */
+        unsigned long long tk = 0, pub = 0;
+        if (lane == 0) {
+            const uint4 v = ld_volatile_v4(g_ticket);
+            tk = ((unsigned long long)v.y << 32) | v.x;
+            pub = ((unsigned long long)v.w << 32) | v.z;
+        }
+        tk = __shfl_sync(0xffffffffu, tk, 0);
+        pub = __shfl_sync(0xffffffffu, pub, 0);
+
+        /* 1. reserve tickets: as many as are visibly waiting, capped by the free slots.  An idle
+         *    CTA of the persistent engine also keeps ONE reservation on a ticket that does not
+         *    exist yet, so that a lone request finds 148 CTAs waiting, one ticket each.         */
+        unsigned long long avail = pub > tk ? pub - tk : 0ull;
+        if (persistent && busy_mask == 0u && have_mask == 0u && avail == 0ull) avail = 1ull;
+        uint32_t n_need = __popc(need);
+        if ((unsigned long long)n_need > avail) {
+            n_need = (uint32_t)avail;
+            need = n_need ? (need & ((2u << (__fns(need, 0, n_need) & 31)) - 1u)) : 0u; /* lowest n_need bits set in need */
+        }
+        if (need) {
+            unsigned long long base = 0;
+            if (lane == 0) base = atomicAdd(g_ticket, (unsigned long long)n_need);
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if ((need >> lane) & 1u) {
+                t = base + __popc(need & ((1u << lane) - 1u));
+                have = true;
+            }
+        }
+
+        /* 2. tickets that have been published by now */
+        if (!persistent && have && t >= P.drain_total) have = false; /* reserved past the end of the queue */
+        const bool ready = have && t < pub; /* pub was read before the reservation: a lower bound */
+        const uint32_t ready_mask = __ballot_sync(0xffffffffu, ready);
+        if (ready_mask) {
+            __threadfence(); /* acquire: the dispatcher's tmap/dq writes precede its store to `published` */
+            unsigned long long entry = 0;
+            if (ready) entry = __ldcg(reinterpret_cast<const unsigned long long *>(P.tmap) + (t & (unsigned long long)(P.TM - 1)));
+            const unsigned long long seq = entry >> AESOFF_TICKET_CHUNK_BITS;
+            const uint32_t chunk = (uint32_t)(entry & ((1u << AESOFF_TICKET_CHUNK_BITS) - 1u));
+            const uint32_t ring = (uint32_t)((seq - 1) & (P.R - 1));
+            /* descriptors: 20 lanes x 16 B each, one slot after the other */
+            for (uint32_t m = ready_mask; m; m &= m - 1u) {
+                const uint32_t sj = __ffs(m) - 1;
+                const uint32_t rj = __shfl_sync(0xffffffffu, ring, sj);
+                if (lane < AESOFF_DESC_BYTES / 16) {
+                    const uint4 v = __ldcg(reinterpret_cast<const uint4 *>(P.dq + rj) + lane);
+                    reinterpret_cast<uint4 *>(&c->slot[sj].desc)[lane] = v;
                 }
-                if (!stop) e = __ldcg(P.tmap + (t & (P.TM - 1)));
             }
-            g->entry = e;
-        }
-        group_sync(group);
-        const unsigned long long e = g->entry;
-        if (e == ENTRY_EXIT) break;
-        const unsigned long long seq = e >> AESOFF_TICKET_CHUNK_BITS;
-        const uint32_t chunk = (uint32_t)(e & ((1u << AESOFF_TICKET_CHUNK_BITS) - 1u));
-        const uint32_t slot = (uint32_t)((seq - 1) & (P.R - 1));
-        if (seq != cached_seq) {
-            /* 320-byte descriptor -> this group's shared memory (20 x 16 B, L2 reads).  Nobody still
-             * reads the previous one: every thread has passed the barrier that ended its last chunk. */
-            if (gtid < AESOFF_DESC_BYTES / 16) {
-                const uint4 v = __ldcg(reinterpret_cast<const uint4 *>(P.dq + slot) + gtid);
-                reinterpret_cast<uint4 *>(&g->desc)[gtid] = v;
+            __syncwarp();
+            if (ready) {
+                Slot *sl = &c->slot[lane];
+                const unsigned long long rows = sl->desc.rows;
+                const uint32_t crows = sl->desc.chunk_rows;
+                const unsigned long long row0 = (unsigned long long)chunk * crows;
+                const uint32_t nrows = (uint32_t)((rows - row0) < crows ? (rows - row0) : crows);
+                const uint32_t fine = sl->desc.flags & AESOFF_FLAG_FINE;
+                const uint32_t n_units = fine ? nrows * 8u : nrows;
+                sl->unit0_row = (uint32_t)row0;
+                sl->ring_slot = ring;
+                sl->n_units = n_units;
+                sl->fine = fine;
+                c->done[lane] = 0u;
+                c->stamp[lane] = stamp_base + __popc(ready_mask & ((1u << lane) - 1u));
+                c->busy[lane] = 1u;
+                __threadfence_block();
+                sts_volatile(&c->claim[lane], n_units << 16); /* open the slot */
+                have = false;
             }
-            cached_seq = seq;
+            stamp_base += __popc(ready_mask);
+            continue;
         }
-        group_sync(group);
-        process_chunk(g, ybase, chunk, warp_in_group, lane);
-        group_sync(group); /* all of this chunk's stores are ordered before the leader's fence */
-        if (gtid == 0) {
-            const uint32_t nchunks = g->desc.nchunks;
-            __threadfence();
-            const uint32_t d = atomicAdd(P.dq_done + slot, 1u);
-            if (d + 1 == nchunks) {
-                P.dq_done[slot] = 0;
-                __threadfence_system();
-                if (P.hmail) P.hmail[slot] = seq;
-                *reinterpret_cast<volatile uint64_t *>(P.dev_done_seq + slot) = seq;
-            }
+
+        /* 3. nothing to load: time to leave? */
+        if (!persistent) {
+            if (tk >= P.drain_total && busy_mask == 0u && __ballot_sync(0xffffffffu, have) == 0u) break;
+        } else if (busy_mask == 0u) {
+            unsigned long long stop = 0;
+            if (lane == 0) stop = ld_acquire_gpu(reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_STOP));
+            if (__shfl_sync(0xffffffffu, stop, 0) != 0ull) break;
         }
+        if (!need) __nanosleep(100);
     }
+    if (lane == 0) sts_volatile(&c->exit_flag, 1u);
 }
 
 /* ------------------------------------------------------------------------------------------ */
@@ -335,6 +315,7 @@ __device__ void worker_loop(const aesoff_params_t &P, GroupCtl *g, uint32_t ybas
 /* ------------------------------------------------------------------------------------------ */
 __device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
 {
+    unsigned long long *g_idle = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_IDLE);
     unsigned long long *g_published = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_PUBLISHED);
     unsigned long long *g_stop = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_STOP);
     const uint32_t Rm = P.R - 1;
@@ -353,8 +334,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
         const unsigned long long v = ld_acquire_sys(&P.hring[slot].seq);
         if (lane == 0) stop = ld_volatile_u32(P.hctl + AESOFF_CTL_STOP);
         const uint32_t ready = __ballot_sync(0xffffffffu, v == s);
-        uint32_t n = __ffs(~ready) - 1; /* length of the ready prefix; 32 if all ready (ffs(0) = 0 -> -1) */
-        if (ready == 0xffffffffu) n = 32;
+        uint32_t n = (ready == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~ready) - 1); /* length of the ready prefix */
         stop = __shfl_sync(0xffffffffu, stop, 0);
         if (n == 0) {
             bool quit = stop != 0;
@@ -382,8 +362,14 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
             reinterpret_cast<uint4 *>(P.dq + sl)[j] = w;
         }
         /* lane k derives the geometry of request next_seq + k */
-        uint32_t nchunks = 0, crows = P.chunk_rows;
+        uint32_t nchunks = 0, crows = P.chunk_rows, fine = 0;
         unsigned long long rows = 0;
+        /* CTAs with nothing to do (kept by the service warps).  While a quarter of the GPU idles, a
+         * request is cut into 1/8-row units so that it spreads over many warps (latency mode).  */
+        unsigned long long idle = 0;
+        if (lane == 0) idle = *reinterpret_cast<volatile unsigned long long *>(g_idle);
+        idle = __shfl_sync(0xffffffffu, idle, 0);
+        const bool gpu_has_room = idle * 4ull >= (unsigned long long)gridDim.x;
         if (lane < n) {
             const uint4 tail = ld_volatile_v4(reinterpret_cast<const uint8_t *>(P.hring + slot) + 272); /* len, nr, flags */
             const uint32_t icb3 = ld_volatile_u32(reinterpret_cast<const volatile uint32_t *>(P.hring[slot].icb + 3));
@@ -391,6 +377,10 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
             const unsigned long long nblocks = (len >> 4) + ((len & 15ull) ? 1ull : 0ull);
             const uint32_t c0 = icb3 >> 24;
             rows = nblocks ? ((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0ull;
+            if (P.fine_rows && rows <= P.fine_rows && (rows <= AESOFF_FINE_ALWAYS_ROWS || gpu_has_room)) {
+                fine = AESOFF_FLAG_FINE;
+                crows = crows > 1u ? crows / 2u : 1u;
+            }
             /* a request must fit the ticket ring with room to spare, and its chunk index 24 bits */
             const unsigned long long max_chunks = P.TM / 4;
             while (((rows + crows - 1) / crows) > max_chunks) crows *= 2;
@@ -425,8 +415,10 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
             __nanosleep(200);
         }
         if (lane >= n) nchunks = 0;
+        __syncwarp(); /* the body copy above (other lanes) precedes the fields written below */
         if (lane < n) {
             aesoff_dev_desc_t *d = P.dq + slot;
+            d->flags = fine;
             d->nchunks = nchunks;
             d->chunk_rows = crows;
             d->seq = s;
@@ -469,28 +461,20 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
     /* tables on a 64 KiB boundary of the shared window so that PRMT can merge base and index */
     const uint32_t tbase = (sbase + 65535u) & ~65535u;
     const uint32_t ctrl = (tbase - sbase >= CTRL_BYTES) ? sbase : tbase + TABLE_BYTES;
+    CtaCtl *c = reinterpret_cast<CtaCtl *>(smem + (ctrl - sbase));
 
-    for (uint32_t idx = tid; idx < 256u * 32u; idx += blockDim.x) {
-        const uint32_t i = idx >> 5, l = idx & 31u;
-        const uint32_t t0 = __ldg(P.T0 + i);
-        const uint32_t a = tbase + i * 256u + l * 4u;
-        sts(a + OFF_T0, t0);
-        sts(a + OFF_T1, rotl32(t0, 8));
-        sts(a + OFF_T2, rotl32(t0, 16));
-        sts(a + OFF_T3, rotl32(t0, 24));
-    }
+    for (uint32_t i = tid; i < CTRL_BYTES / 4; i += blockDim.x) reinterpret_cast<uint32_t *>(c)[i] = 0u;
     if (tid == 0 && blockIdx.x == 0 && P.hctl) P.hctl[AESOFF_CTL_SMEMBASE] = sbase;
-    __syncthreads();
+    fill_tables(tbase, P.T0, tid, blockDim.x); /* ends with __syncthreads() */
 
     const uint32_t warp = tid >> 5, lane = tid & 31u;
-    if (warp == AESOFF_GROUPS_PER_CTA * (AESOFF_GROUP_THREADS / 32)) {
+    if (warp == AESOFF_WORKER_WARPS) {
+        service_loop(P, c, lane);
+    } else if (warp == AESOFF_WORKER_WARPS + 1) {
         if (P.mode == AESOFF_MODE_PERSISTENT && blockIdx.x == 0) dispatcher_loop(P, lane);
-        return;
+    } else {
+        worker_loop(P, c, tbase | (lane * 4u), lane);
     }
-    const int group = (int)(warp / (AESOFF_GROUP_THREADS / 32));
-    GroupCtl *g = reinterpret_cast<GroupCtl *>(smem + (ctrl - sbase)) + group;
-    const uint32_t ybase = tbase | (lane * 4u);
-    worker_loop(P, g, ybase, group, tid - group * AESOFF_GROUP_THREADS);
 }
 
 /* ------------------------------------------------------------------------------------------ */

@@ -194,12 +194,14 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     aes_engine_opts_t o;
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
-    for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 3; ++i)
         if (o.reserved[i]) return fail(AES_E_INVAL);
     if (o.ring_slots == 0) o.ring_slots = 2048;
     if (o.chunk_rows == 0) o.chunk_rows = 4;
     if (!is_pow2(o.ring_slots) || o.ring_slots < 64 || o.ring_slots > 4096) return fail(AES_E_INVAL);
     if (o.chunk_rows > 64) return fail(AES_E_INVAL);
+    if (o.fine_rows == 0) o.fine_rows = 512;
+    if (o.fine_rows == AES_FINE_ROWS_OFF) o.fine_rows = 0;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(AES_E_CUDA);
@@ -269,6 +271,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     p.chunk_rows = e.chunk_rows;
     p.mode = AESOFF_MODE_PERSISTENT;
     p.idle_exit_ms = o.idle_exit_ms;
+    p.fine_rows = o.fine_rows;
     p.first_seq = e.first_seq;
     if (aesoff_launch_engine(&p, e.n_ctas, e.stream) != 0) {
         free_engine_memory(e);
@@ -329,7 +332,7 @@ extern "C" int aes_engine_info(aes_engine_info_t *out)
     out->sm_count = e.sm_count;
     out->n_ctas = e.n_ctas;
     out->threads_per_cta = AESOFF_CTA_THREADS;
-    out->groups_per_cta = AESOFF_GROUPS_PER_CTA;
+    out->worker_warps_per_cta = AESOFF_WORKER_WARPS;
     out->ring_slots = e.R;
     out->chunk_rows = e.chunk_rows;
     out->smem_bytes_per_cta = AESOFF_SMEM_BYTES;
@@ -586,8 +589,11 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     p.chunk_rows = chunk_rows;
     p.mode = AESOFF_MODE_DRAIN;
     p.first_seq = 1;
-    uint64_t ctas = (total + AESOFF_GROUPS_PER_CTA - 1) / AESOFF_GROUPS_PER_CTA;
+    uint64_t total_rows = 0;
+    for (size_t i = 0; i < n; ++i) total_rows += rows[i];
+    uint64_t ctas = (total_rows + AESOFF_ROWS_PER_CTA - 1) / AESOFF_ROWS_PER_CTA;
     if (ctas > (uint64_t)sms) ctas = (uint64_t)sms;
+    if (ctas == 0) ctas = 1;
     if (aesoff_launch_engine(&p, (int)ctas, stream) != 0) return fail(AES_E_CUDA);
     g_kernel_launches.fetch_add(1);
     return AES_OK;

@@ -17,9 +17,12 @@
 
 #define AESOFF_ROW_BLOCKS      256u   /* counter values per row: one value of the low counter byte each */
 #define AESOFF_ROW_BYTES       4096u
-#define AESOFF_GROUP_THREADS   128u   /* one worker group = 4 warps, one per SM sub-partition            */
-#define AESOFF_GROUPS_PER_CTA  4u
-#define AESOFF_CTA_THREADS     (AESOFF_GROUP_THREADS * AESOFF_GROUPS_PER_CTA + 32u) /* + service warp   */
+#define AESOFF_WORKER_WARPS    16u    /* warps that run the cipher; 4 per SM sub-partition               */
+#define AESOFF_SLOTS           16u    /* chunk tickets a CTA holds in shared memory (open + prefetched)   */
+#define AESOFF_CTA_THREADS     ((AESOFF_WORKER_WARPS + 2u) * 32u) /* + service warp + dispatcher warp      */
+#define AESOFF_ROWS_PER_CTA    16u    /* drain mode: one CTA per this many rows of work, up to the SM count */
+#define AESOFF_FLAG_FINE       1u     /* descriptor flag: units of 1/8 row (32 blocks) instead of a row   */
+#define AESOFF_FINE_ALWAYS_ROWS 16u   /* requests up to 64 KiB are always cut fine (submission-bound)     */
 #define AESOFF_BODY_BYTES      288u
 #define AESOFF_DESC_BYTES      320u
 #define AESOFF_TICKET_CHUNK_BITS 24u
@@ -34,11 +37,12 @@
 #define AESOFF_CTL_SMEMBASE    2      /* device -> host: shared-window offset of dynamic smem (debug) */
 #define AESOFF_CTL_WORDS       16
 
-/* device counters, one 128-byte line each (index in uint64 units) */
-#define AESOFF_CNT_TICKET      0
-#define AESOFF_CNT_PUBLISHED   16
-#define AESOFF_CNT_STOP        32
-#define AESOFF_CNT_WORDS       64
+/* device counters (index in uint64 units) */
+#define AESOFF_CNT_TICKET      0      /* next ticket to hand out (atomicAdd by the service warps)      */
+#define AESOFF_CNT_PUBLISHED   1      /* tickets the dispatcher has published; same 16 B as TICKET      */
+#define AESOFF_CNT_IDLE        8      /* CTAs of the persistent engine that have no open slot           */
+#define AESOFF_CNT_STOP        16
+#define AESOFF_CNT_WORDS       32
 
 typedef struct __attribute__((aligned(128))) aesoff_host_slot {
     uint32_t rk[60];       /*   0: round keys, word c of round r at rk[4r+c], little-endian load of the
@@ -86,7 +90,7 @@ typedef struct aesoff_params {
     uint32_t            chunk_rows;
     uint32_t            mode;
     uint32_t            idle_exit_ms;
-    uint32_t            pad;
+    uint32_t            fine_rows;  /* requests of at most this many rows may be cut into 1/8-row units; 0 = never */
     uint64_t            first_seq;  /* sequence number of the first request of this launch */
 } aesoff_params_t;
 

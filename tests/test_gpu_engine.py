@@ -1,5 +1,5 @@
 """-m gpu parity and behaviour of the persistent engine: submission ring -> dispatcher warp ->
-worker groups -> completion mailbox (steps a2, a3, a7 of SURVEY.md section 8(a)), against the
+service warps -> worker warps -> completion mailbox (steps a2, a3, a7 of SURVEY.md section 8(a)), against the
 oracle, byte for byte.
 
 While the engine runs, a device-wide synchronisation would block on the persistent kernel, so these
@@ -15,15 +15,18 @@ from paper_2607_02630_b200 import workloads
 pytestmark = pytest.mark.gpu
 
 
-@pytest.fixture(scope="module")
-def P():
+@pytest.fixture(scope="module", params=["latency_units", "row_units_only"])
+def P(request):
+    """Every test runs twice: with the default unit policy (requests up to 64 KiB, and larger ones
+    that find the GPU idle, are cut into 1/8-row units) and with whole-row units only."""
     import paper_2607_02630_b200.binding as B
     import gpu_util as G
 
     torch = G.torch_cuda()
     torch.zeros(1, device="cuda:0")  # CUDA context + torch's first kernels before the engine occupies the SMs
     torch.cuda.synchronize()
-    B.aes_engine_start(0, idle_exit_ms=60000)
+    B.aes_engine_start(0, idle_exit_ms=60000,
+                       fine_rows=0 if request.param == "latency_units" else B.AES_FINE_ROWS_OFF)
     yield B
     B.aes_engine_stop()
 
