@@ -1,7 +1,7 @@
 /*
  * aesoff_cipher.cuh -- the AES-CTR arithmetic of the sm_100a path (steps a4-a6 of SURVEY.md
  * section 8(a)): shared-memory table layout, table fill, and one "row" of CTR by one warp.
- * Included by aesoff_kernels.cu (engine kernel) and aesoff_calib.cu (calibration kernels).
+ * Included by aesoff_kernels.cu (engine kernel).
  *
  *   FIPS-197 Cipher() with the SubBytes/ShiftRows/MixColumns of a round folded into four
  *   256-entry word tables (the classical "T-table" form of sec. 5.1: column j of a round's output
@@ -98,6 +98,43 @@ __device__ __forceinline__ void fill_tables(uint32_t tbase, const uint32_t *T0, 
         sts(a + OFF_T3, rotl32(t0, 24));
     }
     __syncthreads();
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* key expansion (step a1) for keys that arrive raw in a descriptor: FIPS-197 sec. 5.2          */
+/* ------------------------------------------------------------------------------------------ */
+/* SubWord out of this lane's replica of T0: S[x] is byte 1 (and 2) of T0[x].                   */
+__device__ __forceinline__ uint32_t sub_word(uint32_t w, uint32_t ybase)
+{
+    const uint32_t t0 = TL(0, 0, w), t1 = TL(0, 1, w), t2 = TL(0, 2, w), t3 = TL(0, 3, w);
+    return ((t0 >> 8) & 0xffu) | (t1 & 0xff00u) | (t2 & 0xff0000u) | ((t3 << 16) & 0xff000000u);
+}
+/* key: Nk little-endian-loaded words of the cipher key; out: 4 (Nk + 7) words in global memory.
+ * Words are little-endian loads of the FIPS-197 byte string, so RotWord is a right rotation by 8
+ * and Rcon lands in the low byte.  One thread, one serial chain of Nk + 6 (Nk = 4) or 2 x 7 - 1
+ * (Nk = 8) SubWords: well under a microsecond, against a PCIe round trip for shipping 240 bytes. */
+template <int NK>
+__device__ __noinline__ void key_expand(uint32_t ybase, const uint32_t *key, uint32_t *out)
+{
+    uint32_t w[NK];
+#pragma unroll
+    for (int i = 0; i < NK; ++i) {
+        w[i] = key[i];
+        __stcg(out + i, w[i]);
+    }
+    uint32_t rcon = 1;
+#pragma unroll
+    for (int i = NK; i < 4 * (NK + 7); ++i) {
+        uint32_t t = w[(i - 1) % NK];
+        if (i % NK == 0) {
+            t = sub_word(__funnelshift_r(t, t, 8), ybase) ^ rcon;
+            rcon = ((rcon << 1) ^ ((rcon & 0x80u) ? 0x11bu : 0u)) & 0xffu; /* xtime, sec. 4.2.1 */
+        } else if (NK > 6 && i % NK == 4) {
+            t = sub_word(t, ybase);
+        }
+        w[i % NK] ^= t;
+        __stcg(out + i, w[i % NK]);
+    }
 }
 
 /* ------------------------------------------------------------------------------------------ */

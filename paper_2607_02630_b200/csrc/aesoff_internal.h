@@ -6,10 +6,24 @@
 
 #include "aesoff_shared.h"
 
+/* How a context's key reaches the device (aesoff_runtime.cpp, aes_ctr_submit):
+ *   first submit        the raw key rides in the descriptor, the dispatcher expands it (one-shot
+ *                       contexts, BASELINE.json configs[3], never own device state)
+ *   second submit       as above, and the dispatcher also stores the expanded key at ktab[id]
+ *   later submits       the descriptor only names ktab[id]                                       */
+#define AESOFF_CTX_FRESH      0u
+#define AESOFF_CTX_SEEN       1u
+#define AESOFF_CTX_INSTALLING 2u
+#define AESOFF_CTX_INSTALLED  3u
+
 struct aes_ctx {
-    uint32_t rk[60]; /* round keys as little-endian-loaded words, zero padded */
+    uint32_t rk[60]; /* round keys as little-endian-loaded words, zero padded (host expansion) */
     int32_t nr;      /* 10 or 14 */
     int32_t keybits;
+    uint32_t key[8]; /* the cipher key as little-endian-loaded words, zero padded */
+    uint32_t state;  /* AESOFF_CTX_*, accessed atomically */
+    uint32_t id;     /* ktab index once state >= INSTALLING */
+    uint64_t epoch;  /* ktab generation the id belongs to */
 };
 
 const uint32_t *aesoff_T0_table();

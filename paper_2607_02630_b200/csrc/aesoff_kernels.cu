@@ -15,12 +15,12 @@
  *                 over it (aesoff_cipher.cuh).  Workers never wait on global memory except for the
  *                 payload itself: no barriers, no ticket round trips.
  *   warp 16       SERVICE.  Keeps the CTA's AESOFF_SLOTS slots filled: reserves chunk tickets from
- *                 the device-wide ticket counter, waits until the dispatcher has published them,
- *                 copies the 320-byte descriptor (round keys included) into the slot and opens it
- *                 for claiming -- all while the workers are busy with earlier slots.
+ *                 the device-wide ticket counter, polls them until the dispatcher has written them,
+ *                 copies the 96-byte descriptor and the 240-byte expanded key into the slot and opens
+ *                 it for claiming -- all while the workers are busy with earlier slots.
  *   warp 17       DISPATCHER (CTA 0, persistent mode only).  Polls the host-mapped descriptor ring
- *                 over PCIe, copies request bodies into the device queue and cuts each request into
- *                 chunk tickets (step a3).
+ *                 over PCIe (one round trip per batch of up to 32 requests), expands keys that arrive
+ *                 raw (step a1), and cuts each request into chunk tickets (step a3).
  * Completion (step a7): the worker that finishes the last unit of a slot counts the request's chunks
  * down in global memory; the last chunk's finisher fences at system scope and writes the request's
  * sequence number into the host-mapped mailbox.
@@ -35,16 +35,19 @@ using namespace aesoff;
 
 namespace {
 
+constexpr uint32_t AESOFF_STAGE_STRIDE = 36; /* words per staged descriptor: 32 + padding against bank conflicts */
+
 /* ------------------------------------------------------------------------------------------ */
 /* per-CTA control block in shared memory                                                      */
 /* ------------------------------------------------------------------------------------------ */
 struct __align__(16) Slot {
-    aesoff_dev_desc_t desc; /* 320 B: descriptor of the request, round keys included            */
+    aesoff_dev_desc_t desc; /*  96 B: descriptor of the request                                 */
+    uint4 rk4[16];          /* 256 B: its expanded key (ktab entry), one uint4 per round        */
     uint32_t unit0_row;     /* first row of this chunk                                          */
     uint32_t ring_slot;     /* index of the request in dq / mailbox                             */
     uint32_t n_units;
     uint32_t fine;          /* 1: a unit is one k-iteration (32 blocks) of a row, else a row    */
-};                          /* 336 B */
+};                          /* 368 B */
 
 struct __align__(16) CtaCtl {
     Slot slot[AESOFF_SLOTS];
@@ -57,9 +60,12 @@ struct __align__(16) CtaCtl {
     uint32_t busy[AESOFF_SLOTS];  /* 0 free, 1 filled and not yet completed                      */
     uint32_t exit_flag;
     uint32_t pad[3];
+    /* dispatcher (CTA 0): the descriptors of one poll, as read from the host ring */
+    uint32_t stage[32][AESOFF_STAGE_STRIDE];
 };
 constexpr uint32_t CTRL_BYTES = sizeof(CtaCtl);
 constexpr uint32_t CLAIM_EXIT = 0xffffffffu;
+static_assert(CTRL_BYTES <= 32u * 1024u, "control block must fit beside the tables (AESOFF_SMEM_BYTES)");
 
 __device__ __forceinline__ uint32_t lds_volatile(const uint32_t *p)
 {
@@ -80,12 +86,6 @@ __device__ __forceinline__ unsigned long long ld_acquire_gpu(const unsigned long
 __device__ __forceinline__ void st_release_gpu(unsigned long long *p, unsigned long long v)
 {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
-}
-__device__ __forceinline__ unsigned long long ld_acquire_sys(const volatile uint64_t *p)
-{
-    unsigned long long v;
-    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
-    return v;
 }
 __device__ __forceinline__ uint32_t ld_volatile_u32(const volatile uint32_t *p)
 {
@@ -172,7 +172,7 @@ __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase,
         if (got == CLAIM_EXIT) break;
         const uint32_t s = got >> 16, u = got & 0xffffu;
         const Slot *sl = &c->slot[s];
-        const uint4 *rk4 = reinterpret_cast<const uint4 *>(sl->desc.rk);
+        const uint4 *rk4 = sl->rk4;
         const int nr = (int)sl->desc.nr;
         const uint64_t len = sl->desc.len;
         const uint8_t *src = reinterpret_cast<const uint8_t *>(sl->desc.src);
@@ -223,7 +223,13 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
             if (lane == 0) atomicAdd(g_idle, counted_idle ? 1ull : ~0ull);
         }
 
-        /* ticket counter and published count sit in one 16-byte word: one L2 read gives both */
+        /* two independent L2 reads, issued back to back.  (a) The tickets this warp holds: a ticket
+         * is one self-validating 16-byte word, so polling it finds out that it exists and fetches
+         * it in the same access.  (b) Ticket counter and published count, one 16-byte word.       */
+        if (!persistent && have && t >= P.drain_total) have = false; /* reserved past the end of the queue */
+        const bool polled = have;
+        uint4 tv = make_uint4(0, 0, 0, 0);
+        if (polled) tv = ld_volatile_v4(P.tmap + (t & (unsigned long long)(P.TM - 1)));
         unsigned long long tk = 0, pub = 0;
         if (lane == 0) {
             const uint4 v = ld_volatile_v4(g_ticket);
@@ -254,23 +260,22 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
         }
 
         /* 2. tickets that have been published by now */
-        if (!persistent && have && t >= P.drain_total) have = false; /* reserved past the end of the queue */
-        const bool ready = have && t < pub; /* pub was read before the reservation: a lower bound */
+        const bool ready = polled && tv.w == (uint32_t)t + 1u;
         const uint32_t ready_mask = __ballot_sync(0xffffffffu, ready);
         if (ready_mask) {
-            __threadfence(); /* acquire: the dispatcher's tmap/dq writes precede its store to `published` */
-            unsigned long long entry = 0;
-            if (ready) entry = __ldcg(reinterpret_cast<const unsigned long long *>(P.tmap) + (t & (unsigned long long)(P.TM - 1)));
-            const unsigned long long seq = entry >> AESOFF_TICKET_CHUNK_BITS;
-            const uint32_t chunk = (uint32_t)(entry & ((1u << AESOFF_TICKET_CHUNK_BITS) - 1u));
-            const uint32_t ring = (uint32_t)((seq - 1) & (P.R - 1));
-            /* descriptors: 20 lanes x 16 B each, one slot after the other */
+            __threadfence(); /* acquire: the dispatcher's dq/ktab writes precede its ticket stores */
+            const uint32_t ring = tv.x, chunk = tv.y, keyloc = tv.z;
+            /* descriptor (lanes 0..5) and expanded key (lanes 8..22), 16 B each, one slot after the other */
             for (uint32_t m = ready_mask; m; m &= m - 1u) {
                 const uint32_t sj = __ffs(m) - 1;
                 const uint32_t rj = __shfl_sync(0xffffffffu, ring, sj);
+                const uint32_t kj = __shfl_sync(0xffffffffu, keyloc, sj);
                 if (lane < AESOFF_DESC_BYTES / 16) {
                     const uint4 v = __ldcg(reinterpret_cast<const uint4 *>(P.dq + rj) + lane);
                     reinterpret_cast<uint4 *>(&c->slot[sj].desc)[lane] = v;
+                } else if (lane >= 8 && lane < 8 + 15) {
+                    const uint4 v = __ldcg(reinterpret_cast<const uint4 *>(P.ktab + kj) + (lane - 8));
+                    c->slot[sj].rk4[lane - 8] = v;
                 }
             }
             __syncwarp();
@@ -313,7 +318,11 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
 /* ------------------------------------------------------------------------------------------ */
 /* dispatcher warp (persistent mode, CTA 0): host ring -> device queue + tickets  (a3)         */
 /* ------------------------------------------------------------------------------------------ */
-__device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
+/* One iteration = ONE PCIe round trip: the warp reads the next 8 (quiet) or 32 (busy) ring slots,
+ * 128 B each, as 16-byte pieces that validate themselves (aesoff_shared.h), so there is no
+ * flag-then-body dependency.  Everything after that is on-chip or L2: geometry, key expansion
+ * for raw keys, descriptor and ticket stores, one release of the published count.             */
+__device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase, uint32_t lane)
 {
     unsigned long long *g_idle = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_IDLE);
     unsigned long long *g_published = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_PUBLISHED);
@@ -322,20 +331,58 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
     unsigned long long next_seq = P.first_seq; /* next sequence number to take from the ring   */
     unsigned long long published = 0;          /* tickets published so far                     */
     unsigned long long oldest = P.first_seq;   /* every seq below this is known to be complete */
+    unsigned long long base = 0;               /* first ticket of request `oldest` at the last scan */
     unsigned long long last_activity = globaltimer_ns();
+    uint32_t wide = 0;                         /* 0: poll 8 slots, 1: poll 32                  */
 
     if (lane == 0) P.hctl[AESOFF_CTL_ALIVE] = 1;
 
     for (;;) {
-        /* phase 1: one PCIe round trip looks at the next 32 slots and at the stop word */
+        /* ---- phase 1: the PCIe round trip ---------------------------------------------------- */
+        /* piece g = 32 j + lane of the poll: slot g / 8 after next_seq, piece g % 8 of that slot */
+        uint4 pc[8];
+        const uint32_t nload = wide ? 8u : 2u;
+#pragma unroll
+        for (uint32_t j = 0; j < 8; ++j) {
+            pc[j] = make_uint4(0, 0, 0, 0);
+            if (j < nload) {
+                const uint32_t k = j * 4u + (lane >> 3);
+                const uint32_t sl = (uint32_t)((next_seq + k - 1) & Rm);
+                pc[j] = ld_volatile_v4(reinterpret_cast<const uint8_t *>(P.hring + sl) + 16u * (lane & 7u));
+            }
+        }
+        uint32_t stop = 0;
+        unsigned long long idle = 0;
+        if (lane == 0) {
+            stop = ld_volatile_u32(P.hctl + AESOFF_CTL_STOP);
+            idle = *reinterpret_cast<volatile unsigned long long *>(g_idle);
+        }
+#pragma unroll
+        for (uint32_t j = 0; j < 8; ++j) {
+            if (j < nload) {
+                const uint32_t k = j * 4u + (lane >> 3);
+                *reinterpret_cast<uint4 *>(&c->stage[k][4u * (lane & 7u)]) = pc[j];
+            }
+        }
+        __syncwarp();
+        /* lane k looks at slot k of the poll */
         const unsigned long long s = next_seq + lane;
         const uint32_t slot = (uint32_t)((s - 1) & Rm);
-        uint32_t stop = 0;
-        const unsigned long long v = ld_acquire_sys(&P.hring[slot].seq);
-        if (lane == 0) stop = ld_volatile_u32(P.hctl + AESOFF_CTL_STOP);
-        const uint32_t ready = __ballot_sync(0xffffffffu, v == s);
-        uint32_t n = (ready == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~ready) - 1); /* length of the ready prefix */
+        const uint32_t *sw = c->stage[lane];
+        const uint32_t tag = (uint32_t)s;
+        uint32_t kw = 0;
+        bool valid = false;
+        if (lane < nload * 4u) {
+            kw = sw[AESOFF_PW_INDEX(AESOFF_PW_KEY)];
+            valid = sw[3] == tag && sw[7] == tag && sw[11] == tag && sw[15] == tag;
+            if (valid && (kw & AESOFF_KW_RAW))
+                valid = sw[19] == tag && sw[23] == tag && sw[27] == tag && sw[31] == tag;
+        }
+        const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
+        uint32_t n = (vmask == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~vmask) - 1); /* length of the ready prefix */
         stop = __shfl_sync(0xffffffffu, stop, 0);
+        idle = __shfl_sync(0xffffffffu, idle, 0);
+        wide = (n >= 8u) ? 1u : 0u;
         if (n == 0) {
             bool quit = stop != 0;
             if (!quit && P.idle_exit_ms) {
@@ -354,34 +401,31 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
         }
         last_activity = globaltimer_ns();
 
-        /* phase 2: second round trip copies the n bodies (18 x 16 B each) into dq */
-        for (uint32_t i = lane; i < n * (AESOFF_BODY_BYTES / 16); i += 32) {
-            const uint32_t k = i / (AESOFF_BODY_BYTES / 16), j = i % (AESOFF_BODY_BYTES / 16);
-            const uint32_t sl = (uint32_t)((next_seq + k - 1) & Rm);
-            const uint4 w = ld_volatile_v4(reinterpret_cast<const uint8_t *>(P.hring + sl) + 16 * j);
-            reinterpret_cast<uint4 *>(P.dq + sl)[j] = w;
-        }
-        /* lane k derives the geometry of request next_seq + k */
-        uint32_t nchunks = 0, crows = P.chunk_rows, fine = 0;
-        unsigned long long rows = 0;
+        /* ---- phase 2: lane k derives the geometry of request next_seq + k ---------------------- */
+        uint32_t icb[4] = {0, 0, 0, 0};
+        unsigned long long src = 0, dst = 0, len = 0, rows = 0;
+        uint32_t nchunks = 0, crows = P.chunk_rows, fine = 0, nr = 0;
         /* CTAs with nothing to do (kept by the service warps).  While a quarter of the GPU idles, a
          * request is cut into 1/8-row units so that it spreads over many warps (latency mode).  */
-        unsigned long long idle = 0;
-        if (lane == 0) idle = *reinterpret_cast<volatile unsigned long long *>(g_idle);
-        idle = __shfl_sync(0xffffffffu, idle, 0);
         const bool gpu_has_room = idle * 4ull >= (unsigned long long)gridDim.x;
         if (lane < n) {
-            const uint4 tail = ld_volatile_v4(reinterpret_cast<const uint8_t *>(P.hring + slot) + 272); /* len, nr, flags */
-            const uint32_t icb3 = ld_volatile_u32(reinterpret_cast<const volatile uint32_t *>(P.hring[slot].icb + 3));
-            const unsigned long long len = ((unsigned long long)tail.y << 32) | tail.x;
+#define PW(p) sw[AESOFF_PW_INDEX(p)]
+            icb[0] = PW(AESOFF_PW_ICB + 0);
+            icb[1] = PW(AESOFF_PW_ICB + 1);
+            icb[2] = PW(AESOFF_PW_ICB + 2);
+            icb[3] = PW(AESOFF_PW_ICB + 3);
+            src = ((unsigned long long)PW(AESOFF_PW_SRC + 1) << 32) | PW(AESOFF_PW_SRC);
+            dst = ((unsigned long long)PW(AESOFF_PW_DST + 1) << 32) | PW(AESOFF_PW_DST);
+            len = ((unsigned long long)PW(AESOFF_PW_LEN + 1) << 32) | PW(AESOFF_PW_LEN);
+            nr = kw >> 24;
             const unsigned long long nblocks = (len >> 4) + ((len & 15ull) ? 1ull : 0ull);
-            const uint32_t c0 = icb3 >> 24;
+            const uint32_t c0 = icb[3] >> 24;
             rows = nblocks ? ((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0ull;
             if (P.fine_rows && rows <= P.fine_rows && (rows <= AESOFF_FINE_ALWAYS_ROWS || gpu_has_room)) {
                 fine = AESOFF_FLAG_FINE;
                 crows = crows > 1u ? crows / 2u : 1u;
             }
-            /* a request must fit the ticket ring with room to spare, and its chunk index 24 bits */
+            /* a request must fit the ticket ring with room to spare */
             const unsigned long long max_chunks = P.TM / 4;
             while (((rows + crows - 1) / crows) > max_chunks) crows *= 2;
             nchunks = (uint32_t)((rows + crows - 1) / crows);
@@ -393,45 +437,76 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, uint32_t lane)
             const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d);
             if ((int)lane >= d) incl += y;
         }
-        /* ticket-ring capacity: every unfinished ticket must stay within TM of the newest.  */
         const unsigned long long first_ticket = published + incl - nchunks;
+        /* ticket-ring capacity: every unfinished ticket must stay within TM of the newest.  `base`
+         * is only refreshed (32 completion words per L2 round trip) when the cached one says no. */
         for (;;) {
-            unsigned long long base = published;
-            if (lane == 0) {
-                while (oldest < next_seq &&
-                       *reinterpret_cast<volatile uint64_t *>(P.dev_done_seq + ((oldest - 1) & Rm)) >= oldest)
-                    ++oldest;
-                if (oldest < next_seq)
-                    base = *reinterpret_cast<volatile uint64_t *>(&P.dq[(oldest - 1) & Rm].pad);
-            }
-            base = __shfl_sync(0xffffffffu, base, 0);
             const uint32_t fits = __ballot_sync(0xffffffffu, lane >= n || first_ticket + nchunks - base <= P.TM);
             uint32_t nfit = (fits == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~fits) - 1);
             if (nfit > n) nfit = n;
-            if (nfit > 0) {
-                n = nfit;
-                break;
+            if (nfit == n) break;
+            for (;;) {
+                const unsigned long long q = oldest + lane;
+                bool fin = false;
+                if (q < next_seq)
+                    fin = *reinterpret_cast<volatile uint64_t *>(P.dev_done_seq + ((q - 1) & Rm)) >= q;
+                const uint32_t fm = __ballot_sync(0xffffffffu, fin);
+                const uint32_t adv = (fm == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~fm) - 1);
+                oldest += adv;
+                if (adv < 32u) break;
             }
-            __nanosleep(200);
+            unsigned long long nb = published;
+            if (lane == 0 && oldest < next_seq)
+                nb = *reinterpret_cast<volatile uint64_t *>(&P.dq[(oldest - 1) & Rm].first_ticket);
+            nb = __shfl_sync(0xffffffffu, nb, 0);
+            if (nb == base) {
+                if (nfit > 0) {
+                    n = nfit;
+                    break;
+                }
+                __nanosleep(200);
+            }
+            base = nb;
         }
         if (lane >= n) nchunks = 0;
-        __syncwarp(); /* the body copy above (other lanes) precedes the fields written below */
+
+        /* ---- phase 3: keys, descriptors, tickets ----------------------------------------------- */
+        uint32_t keyloc = kw & 0xffffu;
+        if (!(kw & AESOFF_KW_RAW) && keyloc >= AESOFF_KEY_IDS) keyloc = AESOFF_KEY_IDS + slot; /* never sent by the host */
+        if (lane < n && (kw & AESOFF_KW_RAW)) {
+            if (!(kw & AESOFF_KW_INSTALL) || keyloc >= AESOFF_KEY_IDS) keyloc = AESOFF_KEY_IDS + slot;
+            uint32_t key[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) key[i] = PW(AESOFF_PW_RAWKEY + i);
+            if (nr == 10)
+                key_expand<4>(ybase, key, P.ktab[keyloc].rk); /* step a1 on the device */
+            else
+                key_expand<8>(ybase, key, P.ktab[keyloc].rk);
+        }
+#undef PW
         if (lane < n) {
             aesoff_dev_desc_t *d = P.dq + slot;
-            d->flags = fine;
-            d->nchunks = nchunks;
-            d->chunk_rows = crows;
-            d->seq = s;
-            d->rows = rows;
-            d->pad = first_ticket;
+            uint4 *d4 = reinterpret_cast<uint4 *>(d);
+            d4[0] = make_uint4(icb[0], icb[1], icb[2], icb[3]);
+            d4[1] = make_uint4((uint32_t)src, (uint32_t)(src >> 32), (uint32_t)dst, (uint32_t)(dst >> 32));
+            d4[2] = make_uint4((uint32_t)len, (uint32_t)(len >> 32), nr, fine);
+            d4[3] = make_uint4(nchunks, crows, (uint32_t)s, (uint32_t)(s >> 32));
+            d4[4] = make_uint4((uint32_t)rows, (uint32_t)(rows >> 32), (uint32_t)first_ticket,
+                               (uint32_t)(first_ticket >> 32));
+            d4[5] = make_uint4(keyloc, 0u, 0u, 0u);
         }
-        /* tickets */
+        __threadfence(); /* descriptors and keys before the tickets that point at them */
+        __syncwarp();
         for (uint32_t k = 0; k < n; ++k) {
             const uint32_t nc = __shfl_sync(0xffffffffu, nchunks, k);
             const unsigned long long ft = __shfl_sync(0xffffffffu, first_ticket, k);
-            const unsigned long long sq = next_seq + k;
-            for (uint32_t c = lane; c < nc; c += 32)
-                P.tmap[(ft + c) & (P.TM - 1)] = (sq << AESOFF_TICKET_CHUNK_BITS) | c;
+            const uint32_t kl = __shfl_sync(0xffffffffu, keyloc, k);
+            const uint32_t rs = (uint32_t)((next_seq + k - 1) & Rm);
+            for (uint32_t ch = lane; ch < nc; ch += 32) {
+                const unsigned long long tno = ft + ch;
+                *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
+                    make_uint4(rs, ch, kl, (uint32_t)tno + 1u);
+            }
         }
         const uint32_t total = __shfl_sync(0xffffffffu, incl, n - 1);
         __threadfence();
@@ -471,7 +546,7 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
     if (warp == AESOFF_WORKER_WARPS) {
         service_loop(P, c, lane);
     } else if (warp == AESOFF_WORKER_WARPS + 1) {
-        if (P.mode == AESOFF_MODE_PERSISTENT && blockIdx.x == 0) dispatcher_loop(P, lane);
+        if (P.mode == AESOFF_MODE_PERSISTENT && blockIdx.x == 0) dispatcher_loop(P, c, tbase | (lane * 4u), lane);
     } else {
         worker_loop(P, c, tbase | (lane * 4u), lane);
     }

@@ -5,7 +5,9 @@
  * submit returns at once, the caller suspends, an executor polls and resumes.
  *
  * Memory-model contract with the kernel (aesoff_kernels.cu):
- *   host: write slot body; release-store slot.seq          GPU: ld.acquire.sys seq; read body
+ *   host: each 16-byte piece of a slot (3 payload words + tag = low half of seq) is written with
+ *         ONE 16-byte store                                GPU: reads pieces with 16-byte loads; a
+ *         descriptor is taken when all its pieces carry the expected tag (one PCIe round trip)
  *   GPU : dst stores; bar; leader fence.sys; store mailbox  host: acquire-load mailbox[slot] >= seq
  * A slot is reused for seq + R only after mailbox[slot] >= seq has been observed by the submitter.
  */
@@ -17,14 +19,25 @@
 #include <time.h>
 
 #include <atomic>
+#include <deque>
 #include <mutex>
 #include <vector>
 
 #if defined(__x86_64__)
 #include <immintrin.h>
 #define CPU_RELAX() _mm_pause()
+/* one 16-byte store: a piece of a ring slot is never seen half written */
+static inline void store_piece(uint32_t *dst, uint32_t a, uint32_t b, uint32_t c, uint32_t tag)
+{
+    _mm_store_si128(reinterpret_cast<__m128i *>(dst), _mm_set_epi32((int)tag, (int)c, (int)b, (int)a));
+}
 #else
 #define CPU_RELAX() ((void)0)
+static inline void store_piece(uint32_t *dst, uint32_t a, uint32_t b, uint32_t c, uint32_t tag)
+{
+    unsigned __int128 v = ((unsigned __int128)tag << 96) | ((unsigned __int128)c << 64) | ((unsigned __int128)b << 32) | a;
+    __atomic_store_n(reinterpret_cast<unsigned __int128 *>(dst), v, __ATOMIC_RELEASE);
+}
 #endif
 
 #include "../../include/aesoff.h"
@@ -57,10 +70,18 @@ struct Engine {
     uint64_t *hmail = nullptr;           /* pinned, mapped */
     uint32_t *hctl = nullptr;            /* pinned, mapped */
     aesoff_dev_desc_t *dq = nullptr;
-    uint64_t *tmap = nullptr, *counters = nullptr, *dev_done_seq = nullptr;
+    aesoff_key_t *ktab = nullptr;
+    aesoff_ticket_t *tmap = nullptr;
+    uint64_t *counters = nullptr, *dev_done_seq = nullptr;
     uint32_t *dq_done = nullptr, *dT0 = nullptr;
     uint64_t first_seq = 1;               /* first sequence number of the current run          */
     std::atomic<uint64_t> next_seq{1};    /* next sequence number to hand out (never reset)    */
+    /* ktab indices for installed contexts.  An index freed while next_seq == s is handed out again
+     * only once next_seq >= s + R: by then every request that could name it has completed (a ring
+     * slot is reused only after its previous request completed).                                  */
+    std::mutex id_mu;
+    std::deque<std::pair<uint32_t, uint64_t>> id_free; /* (index, next_seq when freed), FIFO   */
+    std::atomic<uint64_t> k_epoch{1};     /* bumped whenever ktab is (re)allocated             */
 };
 
 Engine g_eng;
@@ -79,6 +100,7 @@ void free_engine_memory(Engine &e)
     if (e.hctl) cudaFreeHost(e.hctl);
     if (e.dq) cudaFree(e.dq);
     if (e.tmap) cudaFree(e.tmap);
+    if (e.ktab) cudaFree(e.ktab);
     if (e.counters) cudaFree(e.counters);
     if (e.dev_done_seq) cudaFree(e.dev_done_seq);
     if (e.dq_done) cudaFree(e.dq_done);
@@ -88,9 +110,35 @@ void free_engine_memory(Engine &e)
     e.hmail = nullptr;
     e.hctl = nullptr;
     e.dq = nullptr;
-    e.tmap = e.counters = e.dev_done_seq = nullptr;
+    e.tmap = nullptr;
+    e.ktab = nullptr;
+    e.counters = e.dev_done_seq = nullptr;
     e.dq_done = e.dT0 = nullptr;
     e.stream = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(e.id_mu);
+        e.k_epoch.fetch_add(1);
+        e.id_free.clear();
+    }
+}
+
+void reset_key_ids(Engine &e)
+{
+    std::lock_guard<std::mutex> lk(e.id_mu);
+    e.k_epoch.fetch_add(1);
+    e.id_free.clear();
+    for (uint32_t i = 0; i < AESOFF_KEY_IDS; ++i) e.id_free.emplace_back(i, 0ull);
+}
+
+/* a ktab index for a context, or AESOFF_KEY_NONE when none may be handed out right now */
+uint32_t alloc_key_id(Engine &e)
+{
+    std::lock_guard<std::mutex> lk(e.id_mu);
+    if (e.id_free.empty()) return AESOFF_KEY_NONE;
+    const auto f = e.id_free.front();
+    if (f.second != 0 && e.next_seq.load(std::memory_order_acquire) < f.second + e.R) return AESOFF_KEY_NONE;
+    e.id_free.pop_front();
+    return f.first;
 }
 
 inline bool is_pow2(uint32_t x) { return x && !(x & (x - 1)); }
@@ -164,10 +212,27 @@ extern "C" aes_ctx_t *aes_ctx_create(const uint8_t *key, int keybits)
     }
     c->nr = aesoff_key_expand(key, keybits, c->rk);
     c->keybits = keybits;
+    memset(c->key, 0, sizeof(c->key));
+    for (int i = 0; i < keybits / 32; ++i)
+        c->key[i] = (uint32_t)key[4 * i] | ((uint32_t)key[4 * i + 1] << 8) | ((uint32_t)key[4 * i + 2] << 16) |
+                    ((uint32_t)key[4 * i + 3] << 24);
+    c->state = AESOFF_CTX_FRESH;
+    c->id = AESOFF_KEY_NONE;
+    c->epoch = 0;
     return c;
 }
 
-extern "C" void aes_ctx_destroy(aes_ctx_t *ctx) { free(ctx); }
+extern "C" void aes_ctx_destroy(aes_ctx_t *ctx)
+{
+    if (!ctx) return;
+    if (__atomic_load_n(&ctx->state, __ATOMIC_ACQUIRE) >= AESOFF_CTX_INSTALLING && ctx->id != AESOFF_KEY_NONE) {
+        Engine &e = g_eng;
+        std::lock_guard<std::mutex> lk(e.id_mu);
+        /* requests in flight may still name the index: it rests until they must have completed */
+        if (ctx->epoch == e.k_epoch.load()) e.id_free.emplace_back(ctx->id, e.next_seq.load());
+    }
+    free(ctx);
+}
 
 extern "C" int aes_ctx_round_keys(const aes_ctx_t *ctx, uint8_t *out)
 {
@@ -232,7 +297,8 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     ok = ok && cudaHostAlloc((void **)&e.hmail, (size_t)e.R * 8, hflags) == cudaSuccess;
     ok = ok && cudaHostAlloc((void **)&e.hctl, AESOFF_CTL_WORDS * 4, hflags) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.dq, (size_t)e.R * sizeof(aesoff_dev_desc_t)) == cudaSuccess;
-    ok = ok && cudaMalloc((void **)&e.tmap, (size_t)e.TM * 8) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.tmap, (size_t)e.TM * sizeof(aesoff_ticket_t)) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.ktab, (size_t)(AESOFF_KEY_IDS + e.R) * sizeof(aesoff_key_t)) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.counters, AESOFF_CNT_WORDS * 8) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.dev_done_seq, (size_t)e.R * 8) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.dq_done, (size_t)e.R * 4) == cudaSuccess;
@@ -245,11 +311,14 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     memset(e.hmail, 0, (size_t)e.R * 8);
     ok = ok && cudaMemset(e.dev_done_seq, 0, (size_t)e.R * 8) == cudaSuccess;
     ok = ok && cudaMemcpy(e.dT0, aesoff_T0_table(), 256 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+    if (ok) reset_key_ids(e);
     }
     /* sequence numbers never restart, so stale slot/mailbox values (< first_seq) can never match */
     memset(e.hctl, 0, AESOFF_CTL_WORDS * 4);
     ok = ok && cudaMemsetAsync(e.counters, 0, AESOFF_CNT_WORDS * 8, e.stream) == cudaSuccess;
     ok = ok && cudaMemsetAsync(e.dq_done, 0, (size_t)e.R * 4, e.stream) == cudaSuccess;
+    /* ticket numbers restart from 0 with every launch: no stale ticket may carry a matching tag */
+    ok = ok && cudaMemsetAsync(e.tmap, 0, (size_t)e.TM * sizeof(aesoff_ticket_t), e.stream) == cudaSuccess;
     if (!ok) {
         free_engine_memory(e);
         return fail(AES_E_CUDA);
@@ -261,6 +330,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     p.hmail = e.hmail;
     p.hctl = e.hctl;
     p.dq = e.dq;
+    p.ktab = e.ktab;
     p.tmap = e.tmap;
     p.counters = e.counters;
     p.dq_done = e.dq_done;
@@ -368,25 +438,68 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
         fail(AES_E_STOPPED);
         return 0;
     }
+    /* how the key travels (aesoff_internal.h): raw the first two times, by ktab index afterwards.
+     * Decided BEFORE the sequence number is claimed: a submit that sees INSTALLED then gets a number
+     * above the installing one, and the dispatcher takes requests in sequence order.              */
+    uint32_t kw = ((uint32_t)ctx->nr << 24) | AESOFF_KEY_NONE | AESOFF_KW_RAW;
+    bool installing = false;
+    uint32_t st = __atomic_load_n(&ctx->state, __ATOMIC_ACQUIRE);
+    if (st == AESOFF_CTX_INSTALLED && ctx->epoch == e.k_epoch.load(std::memory_order_acquire)) {
+        kw = ((uint32_t)ctx->nr << 24) | ctx->id;
+    } else if (st == AESOFF_CTX_FRESH) {
+        __atomic_compare_exchange_n(&ctx->state, &st, AESOFF_CTX_SEEN, false, __ATOMIC_ACQ_REL, __ATOMIC_ACQUIRE);
+    } else if (st == AESOFF_CTX_SEEN || st == AESOFF_CTX_INSTALLED) {
+        /* INSTALLED under an older ktab generation (the engine was rebuilt): install again */
+        const uint32_t id = alloc_key_id(e);
+        if (id != AESOFF_KEY_NONE) {
+            if (__atomic_compare_exchange_n(&ctx->state, &st, AESOFF_CTX_INSTALLING, false, __ATOMIC_ACQ_REL,
+                                            __ATOMIC_ACQUIRE)) {
+                ctx->id = id;
+                ctx->epoch = e.k_epoch.load(std::memory_order_acquire);
+                kw |= AESOFF_KW_INSTALL;
+                kw = (kw & ~0xffffu) | id;
+                installing = true;
+            } else {
+                std::lock_guard<std::mutex> lk(e.id_mu); /* another thread got there first */
+                e.id_free.emplace_front(id, 0ull);
+            }
+        }
+    }
     /* claim the next sequence number, but only if its slot has been vacated */
     uint64_t s = e.next_seq.load(std::memory_order_acquire);
     for (;;) {
         if (s - e.first_seq >= e.R &&
             __atomic_load_n(&e.hmail[(s - 1) & e.Rm], __ATOMIC_ACQUIRE) < s - e.R) {
+            if (installing) { /* undo: the index was never named by a descriptor */
+                {
+                    std::lock_guard<std::mutex> lk(e.id_mu);
+                    e.id_free.emplace_front(ctx->id, 0ull);
+                }
+                ctx->id = AESOFF_KEY_NONE;
+                __atomic_store_n(&ctx->state, AESOFF_CTX_SEEN, __ATOMIC_RELEASE);
+            }
             fail(AES_E_AGAIN);
             return 0;
         }
         if (e.next_seq.compare_exchange_weak(s, s + 1, std::memory_order_acq_rel)) break;
     }
-    aesoff_host_slot_t *slot = &e.hring[(s - 1) & e.Rm];
-    memcpy(slot->rk, ctx->rk, sizeof(slot->rk));
-    memcpy(slot->icb, nonce, 16);
-    slot->src = (uint64_t)(uintptr_t)src;
-    slot->dst = (uint64_t)(uintptr_t)dst;
-    slot->len = (uint64_t)len;
-    slot->nr = (uint32_t)ctx->nr;
-    slot->flags = 0;
-    __atomic_store_n(&slot->seq, s, __ATOMIC_RELEASE);
+    const uint32_t tag = (uint32_t)s;
+    const uint64_t a_src = (uint64_t)(uintptr_t)src, a_dst = (uint64_t)(uintptr_t)dst, a_len = (uint64_t)len;
+    uint32_t icb[4];
+    memcpy(icb, nonce, 16);
+    uint32_t *w = e.hring[(s - 1) & e.Rm].w;
+    if (kw & AESOFF_KW_RAW) { /* second line first: the dispatcher wants it whenever line one says RAW */
+        store_piece(w + 16, ctx->key[0], ctx->key[1], ctx->key[2], tag);
+        store_piece(w + 20, ctx->key[3], ctx->key[4], ctx->key[5], tag);
+        store_piece(w + 24, ctx->key[6], ctx->key[7], 0u, tag);
+        store_piece(w + 28, 0u, 0u, 0u, tag);
+    }
+    store_piece(w + 0, icb[0], icb[1], icb[2], tag);
+    store_piece(w + 4, icb[3], (uint32_t)a_src, (uint32_t)(a_src >> 32), tag);
+    store_piece(w + 8, (uint32_t)a_dst, (uint32_t)(a_dst >> 32), (uint32_t)a_len, tag);
+    store_piece(w + 12, (uint32_t)(a_len >> 32), kw, 0u, tag);
+    /* a later submit may name ktab[id] only after this one, which installs it, has a lower seq */
+    if (installing) __atomic_store_n(&ctx->state, AESOFF_CTX_INSTALLED, __ATOMIC_RELEASE);
     return (aes_handle_t)s;
 }
 
@@ -443,7 +556,9 @@ struct LaunchCtx {
     int device = -1;
     size_t cap_req = 0, cap_tickets = 0; /* capacities (power of two) */
     aesoff_dev_desc_t *dq = nullptr;
-    uint64_t *tmap = nullptr, *counters = nullptr, *dev_done_seq = nullptr;
+    aesoff_key_t *ktab = nullptr;
+    aesoff_ticket_t *tmap = nullptr;
+    uint64_t *counters = nullptr, *dev_done_seq = nullptr;
     uint32_t *dq_done = nullptr, *dT0 = nullptr;
     uint8_t *stage = nullptr; /* pinned */
     size_t stage_bytes = 0;
@@ -504,6 +619,7 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         L.stage_busy = false;
         if (L.dq) cudaFree(L.dq);
         if (L.tmap) cudaFree(L.tmap);
+        if (L.ktab) cudaFree(L.ktab);
         if (L.counters) cudaFree(L.counters);
         if (L.dev_done_seq) cudaFree(L.dev_done_seq);
         if (L.dq_done) cudaFree(L.dq_done);
@@ -513,10 +629,12 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         L.dq = nullptr;
         L.cap_req = R > L.cap_req ? R : L.cap_req;
         L.cap_tickets = TM > L.cap_tickets ? TM : L.cap_tickets;
-        L.stage_bytes = L.cap_req * sizeof(aesoff_dev_desc_t) + L.cap_tickets * 8 + AESOFF_CNT_WORDS * 8;
+        L.stage_bytes = L.cap_req * (sizeof(aesoff_dev_desc_t) + sizeof(aesoff_key_t)) +
+                        L.cap_tickets * sizeof(aesoff_ticket_t) + AESOFF_CNT_WORDS * 8;
         bool ok = true;
         ok = ok && cudaMalloc((void **)&L.dq, L.cap_req * sizeof(aesoff_dev_desc_t)) == cudaSuccess;
-        ok = ok && cudaMalloc((void **)&L.tmap, L.cap_tickets * 8) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.ktab, L.cap_req * sizeof(aesoff_key_t)) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.tmap, L.cap_tickets * sizeof(aesoff_ticket_t)) == cudaSuccess;
         ok = ok && cudaMalloc((void **)&L.counters, AESOFF_CNT_WORDS * 8) == cudaSuccess;
         ok = ok && cudaMalloc((void **)&L.dev_done_seq, L.cap_req * 8) == cudaSuccess;
         ok = ok && cudaMalloc((void **)&L.dq_done, L.cap_req * 4) == cudaSuccess;
@@ -539,12 +657,23 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         L.stage_busy = false;
     }
     aesoff_dev_desc_t *hd = reinterpret_cast<aesoff_dev_desc_t *>(L.stage);
-    uint64_t *ht = reinterpret_cast<uint64_t *>(L.stage + L.cap_req * sizeof(aesoff_dev_desc_t));
-    uint64_t *hc = ht + L.cap_tickets;
+    aesoff_key_t *hk = reinterpret_cast<aesoff_key_t *>(L.stage + L.cap_req * sizeof(aesoff_dev_desc_t));
+    aesoff_ticket_t *ht = reinterpret_cast<aesoff_ticket_t *>(reinterpret_cast<uint8_t *>(hk) + L.cap_req * sizeof(aesoff_key_t));
+    uint64_t *hc = reinterpret_cast<uint64_t *>(ht + L.cap_tickets);
     uint64_t t = 0;
+    size_t nkeys = 0;
     for (size_t i = 0; i < n; ++i) {
+        /* one ktab entry per distinct context of the batch (host-expanded keys, aesoff_keys.cpp) */
+        size_t kl = nkeys;
+        if (i > 0 && ctxs[i] == ctxs[i - 1]) {
+            kl = hd[i - 1].keyloc;
+        } else {
+            memset(&hk[nkeys], 0, sizeof(aesoff_key_t));
+            memcpy(hk[nkeys].rk, ctxs[i]->rk, sizeof(hk[nkeys].rk));
+            ++nkeys;
+        }
         aesoff_dev_desc_t &d = hd[i];
-        memcpy(d.rk, ctxs[i]->rk, sizeof(d.rk));
+        memset(&d, 0, sizeof(d));
         memcpy(d.icb, nonces + 16 * i, 16);
         d.src = (uint64_t)(uintptr_t)srcs[i];
         d.dst = (uint64_t)(uintptr_t)dsts[i];
@@ -555,8 +684,15 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         d.chunk_rows = crows[i];
         d.seq = i + 1;
         d.rows = rows[i];
-        d.pad = t;
-        for (uint32_t c = 0; c < nch[i]; ++c) ht[t + c] = ((uint64_t)(i + 1) << AESOFF_TICKET_CHUNK_BITS) | c;
+        d.first_ticket = t;
+        d.keyloc = (uint32_t)kl;
+        for (uint32_t c = 0; c < nch[i]; ++c) {
+            aesoff_ticket_t &tk = ht[t + c];
+            tk.ring = (uint32_t)i;
+            tk.chunk = c;
+            tk.keyloc = (uint32_t)kl;
+            tk.tag = (uint32_t)(t + c) + 1u;
+        }
         t += nch[i];
     }
     memset(hc, 0, AESOFF_CNT_WORDS * 8);
@@ -564,8 +700,9 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
 
     bool ok = true;
     ok = ok && cudaMemcpyAsync(L.dq, hd, n * sizeof(aesoff_dev_desc_t), cudaMemcpyHostToDevice, stream) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(L.ktab, hk, nkeys * sizeof(aesoff_key_t), cudaMemcpyHostToDevice, stream) == cudaSuccess;
     if (total)
-        ok = ok && cudaMemcpyAsync(L.tmap, ht, (size_t)total * 8, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+        ok = ok && cudaMemcpyAsync(L.tmap, ht, (size_t)total * sizeof(aesoff_ticket_t), cudaMemcpyHostToDevice, stream) == cudaSuccess;
     ok = ok && cudaMemcpyAsync(L.counters, hc, AESOFF_CNT_WORDS * 8, cudaMemcpyHostToDevice, stream) == cudaSuccess;
     ok = ok && cudaEventRecord(L.stage_free, stream) == cudaSuccess;
     L.stage_busy = true;
@@ -578,6 +715,7 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     aesoff_params_t p;
     memset(&p, 0, sizeof(p));
     p.dq = L.dq;
+    p.ktab = L.ktab;
     p.tmap = L.tmap;
     p.counters = L.counters;
     p.dq_done = L.dq_done;

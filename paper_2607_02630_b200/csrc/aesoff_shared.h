@@ -2,13 +2,19 @@
  * aesoff_shared.h -- structures shared by the host runtime and the sm_100a kernels
  * (internal; the public boundary is include/aesoff.h).
  *
- * Data layout in memory (DESIGN.md section 4):
- *   host ring    pinned, host-mapped, R slots of 384 B.  The host writes the 288-byte
- *                body, then release-stores `seq` (own 64-byte line).     step a2
- *   dq           device memory, R descriptors of 320 B: the body copied by the
- *                dispatcher plus the chunk geometry it derived.           step a3
- *   tmap         device memory ring of 2^k 8-byte tickets (seq << 24 | chunk).
- *   mailbox      pinned, host-mapped, R x 8 B: slot -> last completed seq.  step a7
+ * Data layout in memory (DESIGN.md section 5):
+ *   host ring    pinned, host-mapped, R slots of 128 B = 8 self-validating 16-byte pieces
+ *                (3 payload words + the low 32 bits of the request's sequence number).  The
+ *                host writes each piece with ONE 16-byte store, the dispatcher reads each with
+ *                ONE 16-byte load, so a piece is either the old one or the new one and the whole
+ *                descriptor arrives in a single PCIe round trip (no flag-then-body).   step a2
+ *   dq           device memory, R descriptors of 96 B: the request plus the chunk geometry
+ *                the dispatcher derived.                                               step a3
+ *   ktab         device memory, (AESOFF_KEY_IDS + R) expanded keys of 256 B: entries below
+ *                AESOFF_KEY_IDS belong to contexts that have been installed, the rest to ring
+ *                slots (keys of one-shot contexts, expanded on the device).            step a1
+ *   tmap         device memory ring of 2^k 16-byte tickets {ring slot, chunk, key index, tag}.
+ *   mailbox      pinned, host-mapped, R x 8 B: slot -> last completed seq.             step a7
  */
 #ifndef AESOFF_SHARED_H
 #define AESOFF_SHARED_H
@@ -23,10 +29,11 @@
 #define AESOFF_ROWS_PER_CTA    16u    /* drain mode: one CTA per this many rows of work, up to the SM count */
 #define AESOFF_FLAG_FINE       1u     /* descriptor flag: units of 1/8 row (32 blocks) instead of a row   */
 #define AESOFF_FINE_ALWAYS_ROWS 16u   /* requests up to 64 KiB are always cut fine (submission-bound)     */
-#define AESOFF_BODY_BYTES      288u
-#define AESOFF_DESC_BYTES      320u
-#define AESOFF_TICKET_CHUNK_BITS 24u
-#define AESOFF_SMEM_BYTES      (192u * 1024u)
+#define AESOFF_DESC_BYTES      96u
+#define AESOFF_KEY_BYTES       256u   /* one ktab entry: 60 round-key words + padding                     */
+#define AESOFF_KEY_IDS         4096u  /* ktab entries that installed contexts can own                      */
+#define AESOFF_KEY_NONE        0xffffu
+#define AESOFF_SMEM_BYTES      (200u * 1024u)
 
 #define AESOFF_MODE_PERSISTENT 0u
 #define AESOFF_MODE_DRAIN      1u
@@ -44,42 +51,63 @@
 #define AESOFF_CNT_STOP        16
 #define AESOFF_CNT_WORDS       32
 
+/* ---- host ring slot: 8 pieces of {payload[3], tag}; tag = (uint32_t)seq -------------------- */
+/* payload word p (0..23) of a slot is w[(p / 3) * 4 + p % 3]                                    */
+#define AESOFF_PW_ICB          0      /* 4 words: the 16 counter-block bytes, little-endian loads   */
+#define AESOFF_PW_SRC          4      /* 2 words */
+#define AESOFF_PW_DST          6      /* 2 words */
+#define AESOFF_PW_LEN          8      /* 2 words */
+#define AESOFF_PW_KEY          10     /* key word, see AESOFF_KW_*                                  */
+#define AESOFF_PW_SPARE        11
+#define AESOFF_PW_RAWKEY       12     /* 8 words (second 64-byte line): the cipher key itself       */
+#define AESOFF_PW_WORDS        24
+#define AESOFF_PW_INDEX(p)     (((p) / 3) * 4 + (p) % 3)
+/* key word: bits 0..15 ktab index of the context (AESOFF_KEY_NONE = none), bit 16 raw key present
+ * in the second line (the dispatcher expands it, FIPS-197 sec. 5.2), bit 17 store the expanded key
+ * at the ktab index for later requests, bits 24..31 Nr (10 or 14)                                */
+#define AESOFF_KW_RAW          (1u << 16)
+#define AESOFF_KW_INSTALL      (1u << 17)
+
 typedef struct __attribute__((aligned(128))) aesoff_host_slot {
-    uint32_t rk[60];       /*   0: round keys, word c of round r at rk[4r+c], little-endian load of the
-                                   FIPS-197 byte string (byte 0 of the word = row 0 of column c)      */
-    uint32_t icb[4];       /* 240: the 16 counter-block bytes, same loading                            */
-    uint64_t src;          /* 256 */
-    uint64_t dst;          /* 264 */
-    uint64_t len;          /* 272 */
-    uint32_t nr;           /* 280: 10 or 14                                                            */
-    uint32_t flags;        /* 284 */
-    uint64_t pad0[4];      /* 288 */
-    volatile uint64_t seq; /* 320: valid flag = the request's sequence number, written last            */
-    uint64_t pad1[7];
-} aesoff_host_slot_t;      /* 384 bytes */
+    uint32_t w[32];
+} aesoff_host_slot_t;      /* 128 bytes */
 
 typedef struct __attribute__((aligned(16))) aesoff_dev_desc {
-    uint32_t rk[60];
-    uint32_t icb[4];
-    uint64_t src;
-    uint64_t dst;
-    uint64_t len;
-    uint32_t nr;
-    uint32_t flags;
-    /* written by the dispatcher (or by the host for the launch backend) */
-    uint32_t nchunks;      /* 288 */
-    uint32_t chunk_rows;   /* 292: rows per chunk for this request                                     */
-    uint64_t seq;          /* 296 */
-    uint64_t rows;         /* 304: number of 256-counter rows the request touches                      */
-    uint64_t pad;          /* 312 */
-} aesoff_dev_desc_t;       /* 320 bytes */
+    uint32_t icb[4];       /*  0: the 16 counter-block bytes, little-endian loads                    */
+    uint64_t src;          /* 16 */
+    uint64_t dst;          /* 24 */
+    uint64_t len;          /* 32 */
+    uint32_t nr;           /* 40: 10 or 14                                                             */
+    uint32_t flags;        /* 44: AESOFF_FLAG_*                                                        */
+    uint32_t nchunks;      /* 48 */
+    uint32_t chunk_rows;   /* 52: rows per chunk for this request                                      */
+    uint64_t seq;          /* 56 */
+    uint64_t rows;         /* 64: number of 256-counter rows the request touches                       */
+    uint64_t first_ticket; /* 72 */
+    uint32_t keyloc;       /* 80: ktab index of the expanded key                                       */
+    uint32_t pad[3];
+} aesoff_dev_desc_t;       /* 96 bytes */
+
+typedef struct __attribute__((aligned(16))) aesoff_key {
+    uint32_t rk[60];       /* round keys, word c of round r at rk[4r+c], little-endian load of the
+                              FIPS-197 byte string (byte 0 of the word = row 0 of column c)            */
+    uint32_t pad[4];
+} aesoff_key_t;            /* 256 bytes */
+
+typedef struct __attribute__((aligned(16))) aesoff_ticket {
+    uint32_t ring;         /* index of the request in dq / mailbox                                     */
+    uint32_t chunk;
+    uint32_t keyloc;
+    uint32_t tag;          /* (uint32_t)ticket number + 1; the ring is zeroed at engine start          */
+} aesoff_ticket_t;         /* 16 bytes, written and read as one 128-bit access                         */
 
 typedef struct aesoff_params {
     aesoff_host_slot_t *hring;      /* host-mapped (persistent mode)                     */
     volatile uint64_t  *hmail;      /* host-mapped mailbox, may be NULL in drain mode    */
     volatile uint32_t  *hctl;       /* host-mapped control words, NULL in drain mode     */
     aesoff_dev_desc_t  *dq;
-    uint64_t           *tmap;
+    aesoff_key_t       *ktab;
+    aesoff_ticket_t    *tmap;
     uint64_t           *counters;
     uint32_t           *dq_done;
     uint64_t           *dev_done_seq;
