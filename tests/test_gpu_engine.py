@@ -297,3 +297,54 @@ def test_errors_and_handles(P):
     h = P.aes_ctr_submit(ctx, bytes(16), 0, 0, 0)  # len 0: completes, touches nothing
     P.aes_wait(h)
     P.aes_ctx_destroy(ctx)
+
+
+def test_context_key_paths(P):
+    """How a key reaches the device (aesoff_internal.h): raw in the descriptor and expanded by the dispatcher
+    warp (first and second submit of a context), by key-table index afterwards; indices rest after
+    aes_ctx_destroy and run out -- the context then simply stays on the raw path."""
+    import gpu_util as G
+    from oracle import oracle as o
+
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7600]))
+    data = np.frombuffer(rng.bytes(4096 + 7), dtype=np.uint8)
+    src = G.to_device(data)
+    G.stream_sync()
+    # (a) one context, six submits: raw, raw+install, four by index; both key sizes
+    for keylen in (16, 32):
+        key = rng.bytes(keylen)
+        ctx = P.aes_ctx_create(key)
+        for j in range(6):
+            icb = rng.bytes(16)
+            dst = G.device_empty(len(data))
+            P.aes_wait(P.aes_ctr_submit(ctx, icb, src.data_ptr(), dst.data_ptr(), len(data)))
+            assert dst.cpu().numpy().tobytes() == o.ctr(key, icb, data), "submit %d of a %d-bit context" % (j, 8 * keylen)
+        P.aes_ctx_destroy(ctx)
+    # (b) 5,000 short-lived contexts (more than the key table has indices), three submits each, in flight together
+    small = data[:80]
+    ssrc = G.to_device(small)
+    G.stream_sync()
+    n_ctx, per = 5000, 3
+    dsts = G.device_empty(n_ctx * per * 96)
+    keys, icbs, hs = [], [], []
+    for i in range(n_ctx):
+        key = rng.bytes(16 if i % 2 else 32)
+        ctx = P.aes_ctx_create(key)
+        for j in range(per):
+            icb = rng.bytes(16)
+            while True:
+                try:
+                    hs.append(P.aes_ctr_submit(ctx, icb, ssrc.data_ptr(), dsts.data_ptr() + (i * per + j) * 96, len(small)))
+                    break
+                except P.AesOffError as e:
+                    if e.code != P.AES_E_AGAIN:
+                        raise
+            keys.append(key)
+            icbs.append(icb)
+        P.aes_ctx_destroy(ctx)  # allowed as soon as the last submit has returned
+    for h in hs:
+        P.aes_wait(h)
+    got = dsts.cpu().numpy()
+    wants = G.oracle_many([(k, i, small) for k, i in zip(keys, icbs)])
+    for r, want in enumerate(wants):
+        assert got[r * 96: r * 96 + len(small)].tobytes() == want, "context %d submit %d" % (r // per, r % per)
