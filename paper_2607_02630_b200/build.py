@@ -49,7 +49,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return SO
     tmp = SO + ".%d.tmp" % os.getpid()
-    cmd = [_nvcc()] + NVCC_FLAGS + ["-I", os.path.join(_ROOT, "include"), "-I", CSRC, "-o", tmp]
+    extra = os.environ.get("AESOFF_NVCC_EXTRA", "").split()  # e.g. -DAESOFF_NB=8 for tuning experiments
+    cmd = [_nvcc()] + NVCC_FLAGS + extra + ["-I", os.path.join(_ROOT, "include"), "-I", CSRC, "-o", tmp]
     cmd += ["-x", "cu"] + [os.path.join(CSRC, s) for s in SOURCES]
     cmd += ["-lpthread", "-ldl", "-lrt"]
     proc = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)

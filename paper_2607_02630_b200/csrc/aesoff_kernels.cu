@@ -115,6 +115,7 @@ __device__ __forceinline__ unsigned long long globaltimer_ns()
 /* Takes a unit of the oldest open slot.  Returns slot << 16 | unit, or CLAIM_EXIT.             */
 __device__ __forceinline__ uint32_t claim_unit(CtaCtl *c, uint32_t lane)
 {
+    uint32_t backoff = 32u;
     for (;;) {
         uint32_t w = 0, st = 0;
         if (lane < AESOFF_SLOTS) {
@@ -138,7 +139,9 @@ __device__ __forceinline__ uint32_t claim_unit(CtaCtl *c, uint32_t lane)
             continue;
         }
         if (lds_volatile(&c->exit_flag)) return CLAIM_EXIT;
-        __nanosleep(40);
+        /* an idle worker's polling runs on the very pipe the busy ones are bound by: back off */
+        __nanosleep(backoff);
+        if (backoff < 256u) backoff <<= 1;
     }
 }
 
@@ -184,7 +187,7 @@ __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase,
             ctr_request_row<1>(ybase, rk4, nr, g, src, dst, len, m, lane, u & 7u, (u & 7u) + 1u);
         } else {
             const uint64_t m = (uint64_t)sl->unit0_row + u;
-            ctr_request_row<4>(ybase, rk4, nr, g, src, dst, len, m, lane);
+            ctr_request_row<AESOFF_NB>(ybase, rk4, nr, g, src, dst, len, m, lane);
         }
         __syncwarp();
         if (lane == 0) {
@@ -244,6 +247,26 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
          *    exist yet, so that a lone request finds 148 CTAs waiting, one ticket each.         */
         unsigned long long avail = pub > tk ? pub - tk : 0ull;
         if (persistent && busy_mask == 0u && have_mask == 0u && avail == 0ull) avail = 1ull;
+        /*    A CTA does not hoard: what it holds (unclaimed units of its open slots plus the tickets
+         *    it has reserved, in 1/8-row units) stays near one and a half rows per worker -- enough
+         *    to hide a refill (microseconds against 10 us per row), little enough that the end of a
+         *    burst is not left to the few CTAs that grabbed 16 chunks each.                        */
+        {
+            const uint32_t per_ticket = P.chunk_rows * 8u;
+            uint32_t held = 0;
+            if (mine && !is_free) {
+                const uint32_t w = lds_volatile(&c->claim[lane]);
+                const uint32_t left = (w >> 16) > (w & 0xffffu) ? (w >> 16) - (w & 0xffffu) : 0u;
+                held = c->slot[lane].fine ? left : left * 8u;
+            } else if (have) {
+                held = per_ticket;
+            }
+            held = __reduce_add_sync(0xffffffffu, held);
+            const uint32_t hold_max = AESOFF_WORKER_WARPS * 12u; /* 1.5 rows per worker */
+            unsigned long long cap = held < hold_max ? (hold_max - held + per_ticket - 1u) / per_ticket : 0u;
+            if (cap == 0ull && busy_mask == 0u && have_mask == 0u) cap = 1ull;
+            if (avail > cap) avail = cap;
+        }
         uint32_t n_need = __popc(need);
         if ((unsigned long long)n_need > avail) {
             n_need = (uint32_t)avail;

@@ -551,17 +551,18 @@ extern "C" void aes_host_free(void *p)
 /* launch backend: the paper's mechanism (own stream + event)                      */
 /* ============================================================================================ */
 namespace {
+/* Everything one launch reads travels in ONE host->device copy: a blob of
+ *   counters (256 B) | n descriptors | one expanded key per distinct context | the tickets
+ * staged in pinned memory and mirrored at the same offsets in device memory.                     */
 struct LaunchCtx {
     std::mutex mu;
     int device = -1;
     size_t cap_req = 0, cap_tickets = 0; /* capacities (power of two) */
-    aesoff_dev_desc_t *dq = nullptr;
-    aesoff_key_t *ktab = nullptr;
-    aesoff_ticket_t *tmap = nullptr;
-    uint64_t *counters = nullptr, *dev_done_seq = nullptr;
+    uint8_t *blob = nullptr;             /* device */
+    uint8_t *stage = nullptr;            /* pinned host mirror */
+    size_t blob_bytes = 0;
+    uint64_t *dev_done_seq = nullptr;
     uint32_t *dq_done = nullptr, *dT0 = nullptr;
-    uint8_t *stage = nullptr; /* pinned */
-    size_t stage_bytes = 0;
     cudaEvent_t stage_free = nullptr;
     bool stage_busy = false;
 };
@@ -613,33 +614,27 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     if (total >= (1ull << 30)) return fail(AES_E_INVAL);
     const size_t TM = pow2_at_least((size_t)total);
 
-    /* (re)allocate device queue and pinned staging */
+    /* (re)allocate the device blob and its pinned mirror */
     if (L.device != device || L.cap_req < R || L.cap_tickets < TM) {
         if (L.stage_busy) cudaEventSynchronize(L.stage_free);
         L.stage_busy = false;
-        if (L.dq) cudaFree(L.dq);
-        if (L.tmap) cudaFree(L.tmap);
-        if (L.ktab) cudaFree(L.ktab);
-        if (L.counters) cudaFree(L.counters);
+        if (L.blob) cudaFree(L.blob);
         if (L.dev_done_seq) cudaFree(L.dev_done_seq);
         if (L.dq_done) cudaFree(L.dq_done);
         if (L.dT0) cudaFree(L.dT0);
         if (L.stage) cudaFreeHost(L.stage);
         if (!L.stage_free) cudaEventCreateWithFlags(&L.stage_free, cudaEventDisableTiming);
-        L.dq = nullptr;
+        L.blob = nullptr;
         L.cap_req = R > L.cap_req ? R : L.cap_req;
         L.cap_tickets = TM > L.cap_tickets ? TM : L.cap_tickets;
-        L.stage_bytes = L.cap_req * (sizeof(aesoff_dev_desc_t) + sizeof(aesoff_key_t)) +
-                        L.cap_tickets * sizeof(aesoff_ticket_t) + AESOFF_CNT_WORDS * 8;
+        L.blob_bytes = AESOFF_CNT_WORDS * 8 + L.cap_req * (sizeof(aesoff_dev_desc_t) + sizeof(aesoff_key_t)) +
+                       L.cap_tickets * sizeof(aesoff_ticket_t);
         bool ok = true;
-        ok = ok && cudaMalloc((void **)&L.dq, L.cap_req * sizeof(aesoff_dev_desc_t)) == cudaSuccess;
-        ok = ok && cudaMalloc((void **)&L.ktab, L.cap_req * sizeof(aesoff_key_t)) == cudaSuccess;
-        ok = ok && cudaMalloc((void **)&L.tmap, L.cap_tickets * sizeof(aesoff_ticket_t)) == cudaSuccess;
-        ok = ok && cudaMalloc((void **)&L.counters, AESOFF_CNT_WORDS * 8) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.blob, L.blob_bytes) == cudaSuccess;
         ok = ok && cudaMalloc((void **)&L.dev_done_seq, L.cap_req * 8) == cudaSuccess;
         ok = ok && cudaMalloc((void **)&L.dq_done, L.cap_req * 4) == cudaSuccess;
         ok = ok && cudaMalloc((void **)&L.dT0, 256 * 4) == cudaSuccess;
-        ok = ok && cudaHostAlloc((void **)&L.stage, L.stage_bytes, cudaHostAllocDefault) == cudaSuccess;
+        ok = ok && cudaHostAlloc((void **)&L.stage, L.blob_bytes, cudaHostAllocDefault) == cudaSuccess;
         ok = ok && cudaMemcpy(L.dT0, aesoff_T0_table(), 256 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
         ok = ok && cudaMemset(L.dq_done, 0, L.cap_req * 4) == cudaSuccess;
         ok = ok && cudaMemset(L.dev_done_seq, 0, L.cap_req * 8) == cudaSuccess;
@@ -651,23 +646,21 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         }
         L.device = device;
     }
-    /* the previous call's copies must have left the staging buffer */
+    /* the previous call's copy must have left the staging buffer */
     if (L.stage_busy) {
         cudaEventSynchronize(L.stage_free);
         L.stage_busy = false;
     }
-    aesoff_dev_desc_t *hd = reinterpret_cast<aesoff_dev_desc_t *>(L.stage);
-    aesoff_key_t *hk = reinterpret_cast<aesoff_key_t *>(L.stage + L.cap_req * sizeof(aesoff_dev_desc_t));
-    aesoff_ticket_t *ht = reinterpret_cast<aesoff_ticket_t *>(reinterpret_cast<uint8_t *>(hk) + L.cap_req * sizeof(aesoff_key_t));
-    uint64_t *hc = reinterpret_cast<uint64_t *>(ht + L.cap_tickets);
-    uint64_t t = 0;
+    /* blob layout for this call (every part a multiple of 16 bytes) */
+    const size_t off_dq = AESOFF_CNT_WORDS * 8;
+    const size_t off_key = off_dq + n * sizeof(aesoff_dev_desc_t);
+    uint64_t *hc = reinterpret_cast<uint64_t *>(L.stage);
+    aesoff_dev_desc_t *hd = reinterpret_cast<aesoff_dev_desc_t *>(L.stage + off_dq);
+    aesoff_key_t *hk = reinterpret_cast<aesoff_key_t *>(L.stage + off_key);
     size_t nkeys = 0;
     for (size_t i = 0; i < n; ++i) {
-        /* one ktab entry per distinct context of the batch (host-expanded keys, aesoff_keys.cpp) */
-        size_t kl = nkeys;
-        if (i > 0 && ctxs[i] == ctxs[i - 1]) {
-            kl = hd[i - 1].keyloc;
-        } else {
+        /* one key entry per run of requests with the same context (host-expanded, aesoff_keys.cpp) */
+        if (i == 0 || ctxs[i] != ctxs[i - 1]) {
             memset(&hk[nkeys], 0, sizeof(aesoff_key_t));
             memcpy(hk[nkeys].rk, ctxs[i]->rk, sizeof(hk[nkeys].rk));
             ++nkeys;
@@ -679,31 +672,31 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         d.dst = (uint64_t)(uintptr_t)dsts[i];
         d.len = (uint64_t)lens[i];
         d.nr = (uint32_t)ctxs[i]->nr;
-        d.flags = 0;
         d.nchunks = nch[i];
         d.chunk_rows = crows[i];
         d.seq = i + 1;
         d.rows = rows[i];
-        d.first_ticket = t;
-        d.keyloc = (uint32_t)kl;
+        d.keyloc = (uint32_t)(nkeys - 1);
+    }
+    const size_t off_tk = off_key + nkeys * sizeof(aesoff_key_t);
+    aesoff_ticket_t *ht = reinterpret_cast<aesoff_ticket_t *>(L.stage + off_tk);
+    uint64_t t = 0;
+    for (size_t i = 0; i < n; ++i) {
+        hd[i].first_ticket = t;
         for (uint32_t c = 0; c < nch[i]; ++c) {
             aesoff_ticket_t &tk = ht[t + c];
             tk.ring = (uint32_t)i;
             tk.chunk = c;
-            tk.keyloc = (uint32_t)kl;
+            tk.keyloc = hd[i].keyloc;
             tk.tag = (uint32_t)(t + c) + 1u;
         }
         t += nch[i];
     }
     memset(hc, 0, AESOFF_CNT_WORDS * 8);
     hc[AESOFF_CNT_PUBLISHED] = total;
+    const size_t used = off_tk + (size_t)total * sizeof(aesoff_ticket_t);
 
-    bool ok = true;
-    ok = ok && cudaMemcpyAsync(L.dq, hd, n * sizeof(aesoff_dev_desc_t), cudaMemcpyHostToDevice, stream) == cudaSuccess;
-    ok = ok && cudaMemcpyAsync(L.ktab, hk, nkeys * sizeof(aesoff_key_t), cudaMemcpyHostToDevice, stream) == cudaSuccess;
-    if (total)
-        ok = ok && cudaMemcpyAsync(L.tmap, ht, (size_t)total * sizeof(aesoff_ticket_t), cudaMemcpyHostToDevice, stream) == cudaSuccess;
-    ok = ok && cudaMemcpyAsync(L.counters, hc, AESOFF_CNT_WORDS * 8, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+    bool ok = cudaMemcpyAsync(L.blob, L.stage, used, cudaMemcpyHostToDevice, stream) == cudaSuccess;
     ok = ok && cudaEventRecord(L.stage_free, stream) == cudaSuccess;
     L.stage_busy = true;
     if (!ok) {
@@ -714,10 +707,10 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
 
     aesoff_params_t p;
     memset(&p, 0, sizeof(p));
-    p.dq = L.dq;
-    p.ktab = L.ktab;
-    p.tmap = L.tmap;
-    p.counters = L.counters;
+    p.counters = reinterpret_cast<uint64_t *>(L.blob);
+    p.dq = reinterpret_cast<aesoff_dev_desc_t *>(L.blob + off_dq);
+    p.ktab = reinterpret_cast<aesoff_key_t *>(L.blob + off_key);
+    p.tmap = reinterpret_cast<aesoff_ticket_t *>(L.blob + off_tk);
     p.dq_done = L.dq_done;
     p.dev_done_seq = L.dev_done_seq;
     p.T0 = L.dT0;

@@ -23,7 +23,12 @@
 
 #define AESOFF_ROW_BLOCKS      256u   /* counter values per row: one value of the low counter byte each */
 #define AESOFF_ROW_BYTES       4096u
+#ifndef AESOFF_WORKER_WARPS
 #define AESOFF_WORKER_WARPS    16u    /* warps that run the cipher; 4 per SM sub-partition               */
+#endif
+#ifndef AESOFF_NB
+#define AESOFF_NB              4      /* blocks a lane keeps in flight through the rounds (row units)     */
+#endif
 #define AESOFF_SLOTS           16u    /* chunk tickets a CTA holds in shared memory (open + prefetched)   */
 #define AESOFF_CTA_THREADS     ((AESOFF_WORKER_WARPS + 2u) * 32u) /* + service warp + dispatcher warp      */
 #define AESOFF_ROWS_PER_CTA    16u    /* drain mode: one CTA per this many rows of work, up to the SM count */
