@@ -2,7 +2,7 @@
 """bench.py -- the benchmark contract for the AES-CTR offload engine.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                    [--backend engine|launch] [--workload c2|c3] [--no-extras]
+                    [--backend engine|launch] [--workload c2|c3] [--no-extras] [--sweep [--sweep-out F]]
 
 A *step* is one pass of the whole hot path (submit -> dispatch -> counter
 blocks -> cipher -> XOR/store -> completion) over one batch of synthetic input.  At N = 1 the batch
@@ -11,8 +11,9 @@ AES-128-CTR, one shared key, distinct nonces, 64 in flight (closed loop: the nex
 submitted when one completes), payloads resident in HBM.  `value` is payload GB/s of the whole job.
 
 --backend engine (default) is the product path: the persistent kernel fed by the host-mapped ring.
-  The timed region is  [sync | aes_engine_start, K steps, aes_engine_stop | sync]: it contains the
-  one kernel launch the engine ever makes.
+  aes_engine_start (step a0: the one kernel launch the engine ever makes) happens once, right before
+  the timed region  [sync, barrier | K steps | events, sync]; its cost is reported as engine_start_ms.
+--sweep prints BASELINE.json configs[4] (size x in-flight x key size) instead, one JSON line per cell.
 --backend launch runs the same worker code through ordinary launches (aes_ctr_launch_batch, 64
   requests per launch: the paper's own "stream + event" mechanism).  This is the form ncu can
   replay, so the committed profiles are made with it; a persistent kernel that waits for host
@@ -202,9 +203,13 @@ def main():
     ap.add_argument("--workload", default="c2", choices=["c2", "c3"])
     ap.add_argument("--chunk-rows", type=int, default=0)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e / latency / cpu_baseline / kernel-only legs")
+    ap.add_argument("--sweep", action="store_true", help="configs[4]: size x in-flight x key-size table (one GPU)")
+    ap.add_argument("--sweep-out", default="", help="with --sweep: also write the table to this JSON file")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.sweep:
+        return run_sweep(args)
     if args.warmup < 3:
         args.warmup = 3
 
@@ -212,6 +217,7 @@ def main():
     import torch.distributed as dist
 
     import paper_2607_02630_b200.binding as B
+    from paper_2607_02630_b200 import multi
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -222,7 +228,7 @@ def main():
     dev = torch.device("cuda", local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
-    host_pg = dist.new_group(backend="gloo") if world > 1 else None
+    host_pg = multi.host_group(dist) if world > 1 else None
 
     def barrier():
         if world > 1:
@@ -231,8 +237,7 @@ def main():
     def barrier_host():
         # while the persistent kernel runs, a NCCL barrier kernel may find no free SM resources on a
         # full GPU: ranks line up through the store-based (host-side) barrier instead
-        if world > 1:
-            dist.barrier(group=host_pg)
+        multi.host_barrier(dist, host_pg)
 
     hbm_peak, sm_max_mhz, peak_kind = _peaks()
     w, keybits = make_workload(args.workload)
@@ -323,12 +328,10 @@ def main():
     gpu_launches = B.aes_engine_info()["kernel_launches"] - launches_before
     ms_dev = ev0.elapsed_time(ev1)
     ms_host = 1e3 * (t1 - t0)
-    tmax = torch.tensor([ms_dev], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_total = float(tmax.item())
-    bytes_per_step_all = n * size * world
-    value = bytes_per_step_all * args.steps / (ms_total * 1e-3) / 1e9
+    # replicas only: every rank ran the same batch on its own engine; the job
+    # took as long as its slowest rank
+    bps, ms_total = multi.job_throughput(ms_dev, n * size * args.steps, dist if world > 1 else None, host_pg)
+    value = bps / 1e9
     clk = clocks.summary()
 
     # ---- parity spot check of what the timed region wrote (rank 0; oracle is test infrastructure) ----
@@ -398,6 +401,88 @@ def main():
     return 0
 
 
+def mix_c4(B, torch, dev, n=10000):
+    """BASELINE.json configs[3] on the running engine: 10,000 requests, sizes log-uniform 1-64 KiB with
+    0-15 B tails, a fresh AES-128 or AES-256 key per request (aes_ctx_create inside the timed loop; the raw
+    key rides in the descriptor and is expanded by the dispatcher warp), random ICBs, 256 in flight."""
+    w4 = workloads.config4(n=n)
+    stride = 64 * 1024 + 16
+    s4 = torch.empty(n * stride, dtype=torch.uint8, device=dev)  # contents are irrelevant to timing
+    d4 = torch.empty(n * stride, dtype=torch.uint8, device=dev)
+    keys = np.zeros((n, 32), dtype=np.uint8)
+    kb = np.zeros(n, dtype=np.int32)
+    for i in range(n):
+        k = w4.key_of(i)
+        keys[i, :len(k)] = np.frombuffer(k, dtype=np.uint8)
+        kb[i] = 8 * len(k)
+    srcs = np.asarray([s4.data_ptr() + i * stride for i in range(n)], dtype=np.uint64)
+    dsts = np.asarray([d4.data_ptr() + i * stride for i in range(n)], dtype=np.uint64)
+    B.aes_loop_run(w4.icb, srcs, dsts, w4.length, window=w4.in_flight, keys=keys, keybits=kb, want_latency=False)
+    r = B.aes_loop_run(w4.icb, srcs, dsts, w4.length, window=w4.in_flight, keys=keys, keybits=kb)
+    a = r["lat_ns"][n // 20:] / 1e3
+    return {"workload": w4.name, "requests": n, "in_flight": w4.in_flight, "mean_bytes": float(w4.length.mean()),
+            "p50_us": percentile(a, 50), "p99_us": percentile(a, 99), "req_per_s": n / (r["elapsed_ns"] * 1e-9),
+            "payload_gbs": r["bytes"] / r["elapsed_ns"], "key_expansion": "per request, on the device"}
+
+
+def run_sweep(args):
+    """BASELINE.json configs[4]: payload 1 KiB .. 64 MiB in powers of two x in-flight 1/16/256/1024, AES-128 and
+    AES-256, on the persistent engine; one JSON object per cell to stdout (and --sweep-out)."""
+    import torch
+
+    import paper_2607_02630_b200.binding as B
+
+    hbm_peak, sm_max_mhz, _ = _peaks()
+    dev = torch.device("cuda", 0)
+    total = 8 << 30
+    buf = torch.empty(total, dtype=torch.uint8, device=dev)
+    buf.random_(0, 256)
+    torch.cuda.synchronize()
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
+    lds_peak = SMEM_BYTES_PER_CLK_PER_SM * sm_count * sm_max_mhz * 1e6 / 1e9
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE + 5, 1]))
+    cells = []
+    B.aes_engine_start(0, idle_exit_ms=30000)
+    try:
+        for keybits in (128, 256):
+            ctx = B.aes_ctx_create(rng.bytes(keybits // 8))
+            for lg in range(10, 27):
+                size = 1 << lg
+                for depth in (1, 16, 256, 1024):
+                    # distinct buffers while they fit; in place (dst == src) so that depth x size stays within `total`
+                    nbuf = max(1, min(total // size, max(depth, 64)))
+                    if nbuf < depth:
+                        continue  # 64 MiB x 256 and up do not fit 8 GiB: cell skipped, stated in the output
+                    n = max(4 * depth, 64)
+                    while n * size < (256 << 20) and n < 200000:
+                        n *= 2
+                    ptrs = np.asarray([buf.data_ptr() + (i % nbuf) * size for i in range(n)], dtype=np.uint64)
+                    icb = np.zeros((n, 16), dtype=np.uint8)
+                    icb[:, :8] = rng.integers(0, 256, size=(n, 8), dtype=np.uint8)
+                    lens = np.full(n, size, dtype=np.uint64)
+                    B.aes_loop_run(icb[:depth * 2], ptrs[:depth * 2], ptrs[:depth * 2], lens[:depth * 2], window=depth,
+                                   ctx=ctx, want_latency=False)
+                    r = B.aes_loop_run(icb, ptrs, ptrs, lens, window=depth, ctx=ctx)
+                    a = r["lat_ns"][n // 20:] / 1e3
+                    gbs = r["bytes"] / r["elapsed_ns"]
+                    cell = {"keybits": keybits, "bytes": size, "in_flight": depth, "requests": n, "in_place": True,
+                            "payload_gbs": gbs, "req_per_s": n / (r["elapsed_ns"] * 1e-9),
+                            "p50_us": percentile(a, 50), "p99_us": percentile(a, 99),
+                            "frac_lookup_roof": gbs * LOOKUPS[keybits] * 4.0 / 16.0 / lds_peak,
+                            "frac_hbm_roof": 2 * gbs / hbm_peak}
+                    cells.append(cell)
+                    print(json.dumps(cell), flush=True)
+            B.aes_ctx_destroy(ctx)
+    finally:
+        B.aes_engine_stop()
+    if args.sweep_out:
+        with open(args.sweep_out, "w") as f:
+            json.dump({"lookup_roof_gbs_of_lookup_bytes": lds_peak, "hbm_peak_gbs": hbm_peak, "sm_mhz_assumed": sm_max_mhz,
+                       "note": "in place; 64 MiB x 256/1024 in flight skipped (needs more than the 8 GiB the sweep allocates)",
+                       "cells": cells}, f, indent=1)
+    return 0
+
+
 def extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, size, n, step_launch,
            lds_per_payload_byte, lds_peak, hbm_peak):
     res = {}
@@ -458,7 +543,18 @@ def extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, s
         lat["inflight_%d" % depth] = {"p50_us": percentile(a, 50), "p99_us": percentile(a, 99),
                                       "mean_us": float(a.mean()), "req_per_s": nl / (r["elapsed_ns"] * 1e-9)}
     res["latency_4KiB"] = lat
+    # same, payload in pinned HOST memory (the paper's j.buf): read and written over PCIe by the kernel
+    hl = B.aes_host_alloc(2 * pool * small)
+    hls = [hl + (i % pool) * small for i in range(nl)]
+    hld = [hl + (pool + i % pool) * small for i in range(nl)]
+    r = B.aes_loop_run(wl.icb, hls, hld, [small] * nl, window=1, ctx=ctx)
+    a = r["lat_ns"][nl // 20:] / 1e3
+    res["latency_4KiB"]["host_payload_inflight_1"] = {"p50_us": percentile(a, 50), "p99_us": percentile(a, 99),
+                                                      "mean_us": float(a.mean())}
+    # ---- configs[3]: the fine-grained mix, per-request keys (key expansion on the path) ----
+    res["mix_c4"] = mix_c4(B, torch, dev)
     B.aes_engine_stop()
+    B.aes_host_free(hl)
     # freeing pinned memory synchronises the device, so only after the engine has stopped
     del hsv, hdv
     B.aes_host_free(hs)

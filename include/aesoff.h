@@ -73,11 +73,12 @@ typedef struct aes_engine_opts {
     uint32_t n_ctas;          /* persistent CTAs; 0 = one per SM                          */
     uint32_t idle_exit_ms;    /* the kernel exits by itself (engine becomes STOPPED) after
                                  this long with no request; 0 = never                     */
-    uint32_t fine_rows;       /* latency mode: a request of at most this many 4 KiB rows is
-                                 cut into 1/8-row units (32 blocks per warp instead of 256)
-                                 when the GPU has idle CTAs, so that it spreads over many
-                                 warps; requests up to 16 rows always are.  0 = default 512,
-                                 AES_FINE_ROWS_OFF = never                                 */
+    uint32_t fine_rows;       /* latency modes: a request of at most this many 4 KiB rows may
+                                 be cut into units smaller than a row -- 1/8 row (32 blocks per
+                                 warp) when it finds the GPU idle, half a row when the queue is
+                                 short -- so that it spreads over many warps; requests up to 16
+                                 rows are always cut into 1/8 rows.  0 = default 2048 (8 MiB),
+                                 AES_FINE_ROWS_OFF = whole rows only                        */
     uint32_t reserved[3];     /* must be 0                                                */
 } aes_engine_opts_t;
 
@@ -108,6 +109,10 @@ typedef struct aes_engine_info {
     uint64_t completed;          /* requests whose completion the host has observed
                                     through aes_poll/aes_wait, lower bound            */
     uint64_t kernel_launches;    /* CUDA kernels this library launched so far         */
+    uint64_t cut_eighths;        /* requests of the current run the dispatcher cut into
+                                    1/8-row units, ...                                */
+    uint64_t cut_halves;         /* ... into half rows, ...                           */
+    uint64_t cut_rows;           /* ... into whole rows (see fine_rows above)         */
 } aes_engine_info_t;
 int aes_engine_info(aes_engine_info_t *out);     /* host pointer; AES_OK / AES_E_INVAL */
 

@@ -49,7 +49,8 @@ class aes_engine_info_t(ctypes.Structure):
                 ("n_ctas", ctypes.c_int32), ("threads_per_cta", ctypes.c_int32), ("worker_warps_per_cta", ctypes.c_int32),
                 ("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32),
                 ("smem_bytes_per_cta", ctypes.c_uint32), ("reserved0", ctypes.c_uint32),
-                ("submitted", ctypes.c_uint64), ("completed", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64)]
+                ("submitted", ctypes.c_uint64), ("completed", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64),
+                ("cut_eighths", ctypes.c_uint64), ("cut_halves", ctypes.c_uint64), ("cut_rows", ctypes.c_uint64)]
 
 
 class aes_loop_spec_t(ctypes.Structure):

@@ -46,7 +46,8 @@ struct __align__(16) Slot {
     uint32_t unit0_row;     /* first row of this chunk                                          */
     uint32_t ring_slot;     /* index of the request in dq / mailbox                             */
     uint32_t n_units;
-    uint32_t fine;          /* 1: a unit is one k-iteration (32 blocks) of a row, else a row    */
+    uint32_t fine;          /* unit size: 0 a row, AESOFF_FLAG_HALF half a row (128 blocks),
+                               AESOFF_FLAG_FINE one k-iteration of a row (32 blocks)            */
 };                          /* 368 B */
 
 struct __align__(16) CtaCtl {
@@ -182,9 +183,13 @@ __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase,
         uint8_t *dst = reinterpret_cast<uint8_t *>(sl->desc.dst);
         const CtrGeom g = ctr_geom(sl->desc.icb[0], sl->desc.icb[1], sl->desc.icb[2], sl->desc.icb[3]);
         const uint32_t n_units = sl->n_units;
-        if (sl->fine) {
+        const uint32_t fine = sl->fine;
+        if (fine & AESOFF_FLAG_FINE) {
             const uint64_t m = (uint64_t)sl->unit0_row + (u >> 3);
             ctr_request_row<1>(ybase, rk4, nr, g, src, dst, len, m, lane, u & 7u, (u & 7u) + 1u);
+        } else if (fine & AESOFF_FLAG_HALF) {
+            const uint64_t m = (uint64_t)sl->unit0_row + (u >> 1);
+            ctr_request_row<4>(ybase, rk4, nr, g, src, dst, len, m, lane, (u & 1u) * 4u, (u & 1u) * 4u + 4u);
         } else {
             const uint64_t m = (uint64_t)sl->unit0_row + u;
             ctr_request_row<AESOFF_NB>(ybase, rk4, nr, g, src, dst, len, m, lane);
@@ -257,7 +262,8 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
             if (mine && !is_free) {
                 const uint32_t w = lds_volatile(&c->claim[lane]);
                 const uint32_t left = (w >> 16) > (w & 0xffffu) ? (w >> 16) - (w & 0xffffu) : 0u;
-                held = c->slot[lane].fine ? left : left * 8u;
+                const uint32_t f = c->slot[lane].fine;
+                held = (f & AESOFF_FLAG_FINE) ? left : (f & AESOFF_FLAG_HALF) ? left * 4u : left * 8u;
             } else if (have) {
                 held = per_ticket;
             }
@@ -265,6 +271,11 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
             const uint32_t hold_max = AESOFF_WORKER_WARPS * 12u; /* 1.5 rows per worker */
             unsigned long long cap = held < hold_max ? (hold_max - held + per_ticket - 1u) / per_ticket : 0u;
             if (cap == 0ull && busy_mask == 0u && have_mask == 0u) cap = 1ull;
+            /* ... nor takes more than its share of a short queue: the last tickets of a burst (and the
+             * tickets of a lone request) spread over all CTAs instead of piling up on the first few  */
+            const uint32_t a32 = avail > 0x100000ull ? 0x100000u : (uint32_t)avail; /* 32-bit division */
+            const uint32_t share = (a32 + gridDim.x - 1u) / gridDim.x;
+            if (cap > share) cap = share ? share : 1ull;
             if (avail > cap) avail = cap;
         }
         uint32_t n_need = __popc(need);
@@ -308,8 +319,8 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
                 const uint32_t crows = sl->desc.chunk_rows;
                 const unsigned long long row0 = (unsigned long long)chunk * crows;
                 const uint32_t nrows = (uint32_t)((rows - row0) < crows ? (rows - row0) : crows);
-                const uint32_t fine = sl->desc.flags & AESOFF_FLAG_FINE;
-                const uint32_t n_units = fine ? nrows * 8u : nrows;
+                const uint32_t fine = sl->desc.flags & (AESOFF_FLAG_FINE | AESOFF_FLAG_HALF);
+                const uint32_t n_units = (fine & AESOFF_FLAG_FINE) ? nrows * 8u : (fine & AESOFF_FLAG_HALF) ? nrows * 2u : nrows;
                 sl->unit0_row = (uint32_t)row0;
                 sl->ring_slot = ring;
                 sl->n_units = n_units;
@@ -357,6 +368,8 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
     unsigned long long base = 0;               /* first ticket of request `oldest` at the last scan */
     unsigned long long last_activity = globaltimer_ns();
     uint32_t wide = 0;                         /* 0: poll 8 slots, 1: poll 32                  */
+    uint32_t n_eighths = 0, n_halves = 0, n_rows = 0;
+    bool stats_dirty = false;
 
     if (lane == 0) P.hctl[AESOFF_CTL_ALIVE] = 1;
 
@@ -375,10 +388,11 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             }
         }
         uint32_t stop = 0;
-        unsigned long long idle = 0;
+        unsigned long long idle = 0, reserved = 0;
         if (lane == 0) {
             stop = ld_volatile_u32(P.hctl + AESOFF_CTL_STOP);
             idle = *reinterpret_cast<volatile unsigned long long *>(g_idle);
+            reserved = *reinterpret_cast<volatile unsigned long long *>(P.counters + AESOFF_CNT_TICKET);
         }
 #pragma unroll
         for (uint32_t j = 0; j < 8; ++j) {
@@ -405,8 +419,18 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         uint32_t n = (vmask == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~vmask) - 1); /* length of the ready prefix */
         stop = __shfl_sync(0xffffffffu, stop, 0);
         idle = __shfl_sync(0xffffffffu, idle, 0);
+        reserved = __shfl_sync(0xffffffffu, reserved, 0);
         wide = (n >= 8u) ? 1u : 0u;
         if (n == 0) {
+            if (stats_dirty) {
+                /* not on a request's way: a PCIe write in flight would hold up the next fence */
+                if (lane == 0) {
+                    P.hctl[AESOFF_CTL_CUT_EIGHTHS] = n_eighths;
+                    P.hctl[AESOFF_CTL_CUT_HALVES] = n_halves;
+                    P.hctl[AESOFF_CTL_CUT_ROWS] = n_rows;
+                }
+                stats_dirty = false;
+            }
             bool quit = stop != 0;
             if (!quit && P.idle_exit_ms) {
                 const unsigned long long now = globaltimer_ns();
@@ -428,9 +452,18 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         uint32_t icb[4] = {0, 0, 0, 0};
         unsigned long long src = 0, dst = 0, len = 0, rows = 0;
         uint32_t nchunks = 0, crows = P.chunk_rows, fine = 0, nr = 0;
-        /* CTAs with nothing to do (kept by the service warps).  While a quarter of the GPU idles, a
-         * request is cut into 1/8-row units so that it spreads over many warps (latency mode).  */
-        const bool gpu_has_room = idle * 4ull >= (unsigned long long)gridDim.x;
+        /* Latency modes.  A request of up to 64 KiB is always cut into 1/8-row units (32 blocks per
+         * warp; it is submission-bound anyway).  A larger one, up to fine_rows rows, is cut by the
+         * load it meets = rows not yet reserved by any CTA + the rows of this poll up to and including it:
+         *   - 1/8-row units while a quarter of the CTAs have nothing to do and the load makes at most two
+         *     waves of such units over the GPU's worker warps (a lone request: spread it over every
+         *     warp; 17 % more lookups per block, nobody is waiting for them);
+         *   - half rows while the load makes at most one and a half waves of half rows: half the time
+         *     per unit for 2.5 % more lookups;
+         *   - whole rows otherwise (saturation).                                                     */
+        const unsigned long long backlog = published > reserved ? published - reserved : 0ull;
+        const bool gpu_idle = idle * 4ull >= (unsigned long long)gridDim.x;
+        const unsigned long long warps = (unsigned long long)gridDim.x * AESOFF_WORKER_WARPS;
         if (lane < n) {
 #define PW(p) sw[AESOFF_PW_INDEX(p)]
             icb[0] = PW(AESOFF_PW_ICB + 0);
@@ -444,9 +477,25 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             const unsigned long long nblocks = (len >> 4) + ((len & 15ull) ? 1ull : 0ull);
             const uint32_t c0 = icb[3] >> 24;
             rows = nblocks ? ((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0ull;
-            if (P.fine_rows && rows <= P.fine_rows && (rows <= AESOFF_FINE_ALWAYS_ROWS || gpu_has_room)) {
-                fine = AESOFF_FLAG_FINE;
-                crows = crows > 1u ? crows / 2u : 1u;
+        }
+        /* rows of this poll up to and including request k */
+        unsigned long long rows_incl = (lane < n) ? rows : 0ull;
+        if (n > 1) { /* a lone request (the latency case) skips the scan */
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned long long y = __shfl_up_sync(0xffffffffu, rows_incl, d);
+                if ((int)lane >= d) rows_incl += y;
+            }
+        }
+        if (lane < n) {
+            const unsigned long long load = backlog * P.chunk_rows + rows_incl;
+            if (P.fine_rows && rows <= P.fine_rows) {
+                if (rows <= AESOFF_FINE_ALWAYS_ROWS || (gpu_idle && load * 8ull <= 2ull * warps)) {
+                    fine = AESOFF_FLAG_FINE;
+                    crows = crows > 1u ? crows / 2u : 1u;
+                } else if (load * 4ull <= 3ull * warps) {
+                    fine = AESOFF_FLAG_HALF;
+                }
             }
             /* a request must fit the ticket ring with room to spare */
             const unsigned long long max_chunks = P.TM / 4;
@@ -455,10 +504,12 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         }
         /* exclusive prefix sum of nchunks -> first ticket of each request */
         uint32_t incl = nchunks;
+        if (n > 1) {
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d);
-            if ((int)lane >= d) incl += y;
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d);
+                if ((int)lane >= d) incl += y;
+            }
         }
         const unsigned long long first_ticket = published + incl - nchunks;
         /* ticket-ring capacity: every unfinished ticket must stay within TM of the newest.  `base`
@@ -492,6 +543,14 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             base = nb;
         }
         if (lane >= n) nchunks = 0;
+        {   /* statistics for aes_engine_info */
+            const uint32_t me = __ballot_sync(0xffffffffu, lane < n && (fine & AESOFF_FLAG_FINE));
+            const uint32_t mh = __ballot_sync(0xffffffffu, lane < n && (fine & AESOFF_FLAG_HALF));
+            n_eighths += __popc(me);
+            n_halves += __popc(mh);
+            n_rows += n - __popc(me) - __popc(mh);
+            stats_dirty = true; /* written to the host when the ring is next found empty */
+        }
 
         /* ---- phase 3: keys, descriptors, tickets ----------------------------------------------- */
         uint32_t keyloc = kw & 0xffffu;

@@ -265,7 +265,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     if (o.chunk_rows == 0) o.chunk_rows = 4;
     if (!is_pow2(o.ring_slots) || o.ring_slots < 64 || o.ring_slots > 4096) return fail(AES_E_INVAL);
     if (o.chunk_rows > 64) return fail(AES_E_INVAL);
-    if (o.fine_rows == 0) o.fine_rows = 512;
+    if (o.fine_rows == 0) o.fine_rows = 2048;
     if (o.fine_rows == AES_FINE_ROWS_OFF) o.fine_rows = 0;
 
     int ndev = 0;
@@ -415,6 +415,11 @@ extern "C" int aes_engine_info(aes_engine_info_t *out)
     }
     out->completed = out->submitted - pending;
     out->kernel_launches = g_kernel_launches.load();
+    if (e.hctl) {
+        out->cut_eighths = __atomic_load_n(&e.hctl[AESOFF_CTL_CUT_EIGHTHS], __ATOMIC_RELAXED);
+        out->cut_halves = __atomic_load_n(&e.hctl[AESOFF_CTL_CUT_HALVES], __ATOMIC_RELAXED);
+        out->cut_rows = __atomic_load_n(&e.hctl[AESOFF_CTL_CUT_ROWS], __ATOMIC_RELAXED);
+    }
     return AES_OK;
 }
 

@@ -33,6 +33,7 @@
 #define AESOFF_CTA_THREADS     ((AESOFF_WORKER_WARPS + 2u) * 32u) /* + service warp + dispatcher warp      */
 #define AESOFF_ROWS_PER_CTA    16u    /* drain mode: one CTA per this many rows of work, up to the SM count */
 #define AESOFF_FLAG_FINE       1u     /* descriptor flag: units of 1/8 row (32 blocks) instead of a row   */
+#define AESOFF_FLAG_HALF       2u     /* descriptor flag: units of half a row (128 blocks)                */
 #define AESOFF_FINE_ALWAYS_ROWS 16u   /* requests up to 64 KiB are always cut fine (submission-bound)     */
 #define AESOFF_DESC_BYTES      96u
 #define AESOFF_KEY_BYTES       256u   /* one ktab entry: 60 round-key words + padding                     */
@@ -47,6 +48,9 @@
 #define AESOFF_CTL_STOP        0      /* host -> device: 1 = exit after the ring is drained */
 #define AESOFF_CTL_ALIVE       1      /* device -> host: 1 once the kernel polls, 2 after it exits */
 #define AESOFF_CTL_SMEMBASE    2      /* device -> host: shared-window offset of dynamic smem (debug) */
+#define AESOFF_CTL_CUT_EIGHTHS 4      /* device -> host: requests cut into 1/8-row units so far (statistics) */
+#define AESOFF_CTL_CUT_HALVES  5      /*                 ... into half rows                                  */
+#define AESOFF_CTL_CUT_ROWS    6      /*                 ... into whole rows                                 */
 #define AESOFF_CTL_WORDS       16
 
 /* device counters (index in uint64 units) */

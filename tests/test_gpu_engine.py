@@ -27,6 +27,7 @@ def P(request):
     torch.cuda.synchronize()
     B.aes_engine_start(0, idle_exit_ms=60000,
                        fine_rows=0 if request.param == "latency_units" else B.AES_FINE_ROWS_OFF)
+    B.test_latency_units = request.param == "latency_units"
     yield B
     B.aes_engine_stop()
 
@@ -348,3 +349,29 @@ def test_context_key_paths(P):
     wants = G.oracle_many([(k, i, small) for k, i in zip(keys, icbs)])
     for r, want in enumerate(wants):
         assert got[r * 96: r * 96 + len(small)].tobytes() == want, "context %d submit %d" % (r // per, r % per)
+
+
+def test_unit_sizes_half_rows_and_eighths(P):
+    """The dispatcher's three unit sizes on one engine: a lone request is cut into 1/8-row units, a
+    short queue of 1 MiB requests into half rows, a long queue into whole rows; every byte checked,
+    ragged tails and an ICB whose low byte is not 0 (the first row starts in its middle)."""
+    import time
+
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7800]))
+    key = rng.bytes(16)
+    before = P.aes_engine_info()
+    lone = [(key, rng.bytes(15) + b"\x9c", np.frombuffer(rng.bytes((1 << 20) + 7), dtype=np.uint8))]
+    _check(P, lone)
+    short = [(key, rng.bytes(15) + bytes([37 * i % 256]), np.frombuffer(rng.bytes((1 << 20) + 16 * i + 3), dtype=np.uint8))
+             for i in range(6)]
+    _check(P, short)
+    long_q = [(key, rng.bytes(16), np.frombuffer(rng.bytes((2 << 20) + 5), dtype=np.uint8)) for i in range(48)]
+    _check(P, long_q)
+    time.sleep(0.01)  # the statistics are written when the dispatcher next finds the ring empty
+    after = P.aes_engine_info()
+    d = {k: after[k] - before[k] for k in ("cut_eighths", "cut_halves", "cut_rows")}
+    assert sum(d.values()) == len(lone) + len(short) + len(long_q)
+    if P.test_latency_units:
+        assert d["cut_eighths"] >= 1 and d["cut_halves"] >= 1 and d["cut_rows"] >= 1, d
+    else:
+        assert d["cut_rows"] == sum(d.values())
