@@ -80,24 +80,29 @@ __device__ __noinline__ void store_partial(const uint8_t *src, uint8_t *dst, uin
 /* table fill (step a0): T0 comes from global memory (256 words built by the host from the     */
 /* S-box definition, aesoff_keys.cpp); T1..T3 are its byte rotations; 32 replicas each         */
 /* ------------------------------------------------------------------------------------------ */
-/* All threads of the CTA call this; ends with the tables complete (contains __syncthreads).     */
+/* Called by the CTA's first `nthreads` threads (the worker warps; a multiple of 32); they meet on
+ * named barrier 2, and the tables are complete when it returns.                                 */
+__device__ __forceinline__ void fill_barrier(uint32_t nthreads)
+{
+    asm volatile("bar.sync 2, %0;" ::"r"(nthreads) : "memory");
+}
 __device__ __forceinline__ void fill_tables(uint32_t tbase, const uint32_t *T0, uint32_t tid, uint32_t nthreads)
 {
     /* one global read per entry, staged in what becomes lane 0's replica of T0 ... */
     for (uint32_t i = tid; i < 256u; i += nthreads) sts(tbase + i * 256u + OFF_T0, __ldg(T0 + i));
-    __syncthreads();
+    fill_barrier(nthreads);
     /* ... then replicated and rotated out of shared memory */
     for (uint32_t idx = tid; idx < 256u * 32u; idx += nthreads) {
         const uint32_t i = idx >> 5, l = idx & 31u;
         uint32_t t0;
         asm volatile("ld.shared.u32 %0, [%1];" : "=r"(t0) : "r"(tbase + i * 256u) : "memory");
         const uint32_t a = tbase + i * 256u + l * 4u;
-        sts(a + OFF_T0, t0);
+        if (l != 0u) sts(a + OFF_T0, t0);
         sts(a + OFF_T1, rotl32(t0, 8));
         sts(a + OFF_T2, rotl32(t0, 16));
         sts(a + OFF_T3, rotl32(t0, 24));
     }
-    __syncthreads();
+    fill_barrier(nthreads);
 }
 
 /* ------------------------------------------------------------------------------------------ */

@@ -171,9 +171,19 @@ __device__ __forceinline__ void complete_chunk(const aesoff_params_t &P, CtaCtl 
 
 __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase, uint32_t lane)
 {
+#ifdef AESOFF_DEBUG
+    bool first = true;
+#endif
     for (;;) {
         const uint32_t got = claim_unit(c, lane);
         if (got == CLAIM_EXIT) break;
+#ifdef AESOFF_DEBUG
+        if (lane == 0 && first) {
+            atomicMin(reinterpret_cast<unsigned long long *>(P.counters) + 20 + 3, globaltimer_ns()); /* first unit claimed anywhere */
+            atomicMax(reinterpret_cast<unsigned long long *>(P.counters) + 20 + 4, globaltimer_ns()); /* last warp gets its first unit */
+        }
+        first = false;
+#endif
         const uint32_t s = got >> 16, u = got & 0xffffu;
         const Slot *sl = &c->slot[s];
         const uint4 *rk4 = sl->rk4;
@@ -298,18 +308,40 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
         const uint32_t ready_mask = __ballot_sync(0xffffffffu, ready);
         if (ready_mask) {
             __threadfence(); /* acquire: the dispatcher's dq/ktab writes precede its ticket stores */
-            const uint32_t ring = tv.x, chunk = tv.y, keyloc = tv.z;
-            /* descriptor (lanes 0..5) and expanded key (lanes 8..22), 16 B each, one slot after the other */
-            for (uint32_t m = ready_mask; m; m &= m - 1u) {
-                const uint32_t sj = __ffs(m) - 1;
-                const uint32_t rj = __shfl_sync(0xffffffffu, ring, sj);
-                const uint32_t kj = __shfl_sync(0xffffffffu, keyloc, sj);
-                if (lane < AESOFF_DESC_BYTES / 16) {
-                    const uint4 v = __ldcg(reinterpret_cast<const uint4 *>(P.dq + rj) + lane);
-                    reinterpret_cast<uint4 *>(&c->slot[sj].desc)[lane] = v;
-                } else if (lane >= 8 && lane < 8 + 15) {
-                    const uint4 v = __ldcg(reinterpret_cast<const uint4 *>(P.ktab + kj) + (lane - 8));
-                    c->slot[sj].rk4[lane - 8] = v;
+            const uint32_t ring = tv.x, chunk = tv.y & AESOFF_TICKET_CHUNK_MASK, keyloc = tv.z;
+            const uint32_t unit_mode = tv.y >> AESOFF_TICKET_MODE_SHIFT; /* AESOFF_FLAG_FINE / _HALF / 0 */
+            /* descriptor (lanes 0..5) and expanded key (lanes 8..22), 16 B each; four slots' loads are in
+             * flight together (one L2 round trip per four slots, not per slot)                          */
+            for (uint32_t m = ready_mask; m;) {
+                uint32_t sj[4];
+                uint4 v[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    sj[q] = 32u;
+                    if (m) {
+                        sj[q] = __ffs(m) - 1;
+                        m &= m - 1u;
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (sj[q] < 32u) {
+                        const uint32_t rj = __shfl_sync(0xffffffffu, ring, sj[q]);
+                        const uint32_t kj = __shfl_sync(0xffffffffu, keyloc, sj[q]);
+                        if (lane < AESOFF_DESC_BYTES / 16)
+                            v[q] = __ldcg(reinterpret_cast<const uint4 *>(P.dq + rj) + lane);
+                        else if (lane >= 8 && lane < 8 + 15)
+                            v[q] = __ldcg(reinterpret_cast<const uint4 *>(P.ktab + kj) + (lane - 8));
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (sj[q] < 32u) {
+                        if (lane < AESOFF_DESC_BYTES / 16)
+                            reinterpret_cast<uint4 *>(&c->slot[sj[q]].desc)[lane] = v[q];
+                        else if (lane >= 8 && lane < 8 + 15)
+                            c->slot[sj[q]].rk4[lane - 8] = v[q];
+                    }
                 }
             }
             __syncwarp();
@@ -319,7 +351,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
                 const uint32_t crows = sl->desc.chunk_rows;
                 const unsigned long long row0 = (unsigned long long)chunk * crows;
                 const uint32_t nrows = (uint32_t)((rows - row0) < crows ? (rows - row0) : crows);
-                const uint32_t fine = sl->desc.flags & (AESOFF_FLAG_FINE | AESOFF_FLAG_HALF);
+                const uint32_t fine = unit_mode & (AESOFF_FLAG_FINE | AESOFF_FLAG_HALF);
                 const uint32_t n_units = (fine & AESOFF_FLAG_FINE) ? nrows * 8u : (fine & AESOFF_FLAG_HALF) ? nrows * 2u : nrows;
                 sl->unit0_row = (uint32_t)row0;
                 sl->ring_slot = ring;
@@ -583,11 +615,12 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             const uint32_t nc = __shfl_sync(0xffffffffu, nchunks, k);
             const unsigned long long ft = __shfl_sync(0xffffffffu, first_ticket, k);
             const uint32_t kl = __shfl_sync(0xffffffffu, keyloc, k);
+            const uint32_t md = __shfl_sync(0xffffffffu, fine, k) << AESOFF_TICKET_MODE_SHIFT;
             const uint32_t rs = (uint32_t)((next_seq + k - 1) & Rm);
             for (uint32_t ch = lane; ch < nc; ch += 32) {
                 const unsigned long long tno = ft + ch;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
-                    make_uint4(rs, ch, kl, (uint32_t)tno + 1u);
+                    make_uint4(rs, ch | md, kl, (uint32_t)tno + 1u);
             }
         }
         const uint32_t total = __shfl_sync(0xffffffffu, incl, n - 1);
@@ -620,17 +653,34 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
     const uint32_t ctrl = (tbase - sbase >= CTRL_BYTES) ? sbase : tbase + TABLE_BYTES;
     CtaCtl *c = reinterpret_cast<CtaCtl *>(smem + (ctrl - sbase));
 
-    for (uint32_t i = tid; i < CTRL_BYTES / 4; i += blockDim.x) reinterpret_cast<uint32_t *>(c)[i] = 0u;
-    if (tid == 0 && blockIdx.x == 0 && P.hctl) P.hctl[AESOFF_CTL_SMEMBASE] = sbase;
-    fill_tables(tbase, P.T0, tid, blockDim.x); /* ends with __syncthreads() */
-
+#ifdef AESOFF_DEBUG
+#define DBG_MIN(i) do { if (tid == 0 || (tid & 31u) == 0) atomicMin(reinterpret_cast<unsigned long long *>(P.counters) + 20 + (i), globaltimer_ns()); } while (0)
+#define DBG_MAX(i) do { if (tid == 0 || (tid & 31u) == 0) atomicMax(reinterpret_cast<unsigned long long *>(P.counters) + 20 + (i), globaltimer_ns()); } while (0)
+#else
+#define DBG_MIN(i) ((void)0)
+#define DBG_MAX(i) ((void)0)
+#endif
+    DBG_MIN(0); /* first CTA starts */
+    DBG_MAX(1); /* last CTA starts  */
+    /* Start-up: the worker warps build the tables (named barrier 2 among themselves) while the service
+     * warp clears the control block and already fetches the first tickets; barrier 1 joins the two.  */
     const uint32_t warp = tid >> 5, lane = tid & 31u;
     if (warp == AESOFF_WORKER_WARPS) {
+        for (uint32_t i = lane; i < CTRL_BYTES / 4; i += 32u) reinterpret_cast<uint32_t *>(c)[i] = 0u;
+        __threadfence_block();
+        asm volatile("bar.arrive 1, %0;" ::"n"(AESOFF_CTA_THREADS) : "memory");
         service_loop(P, c, lane);
     } else if (warp == AESOFF_WORKER_WARPS + 1) {
+        asm volatile("bar.sync 1, %0;" ::"n"(AESOFF_CTA_THREADS) : "memory");
         if (P.mode == AESOFF_MODE_PERSISTENT && blockIdx.x == 0) dispatcher_loop(P, c, tbase | (lane * 4u), lane);
     } else {
+        if (tid == 0 && blockIdx.x == 0 && P.hctl) P.hctl[AESOFF_CTL_SMEMBASE] = sbase;
+        fill_tables(tbase, P.T0, tid, AESOFF_WORKER_WARPS * 32u); /* worker threads only */
+        DBG_MAX(2); /* last CTA has its tables */
+        asm volatile("bar.sync 1, %0;" ::"n"(AESOFF_CTA_THREADS) : "memory");
         worker_loop(P, c, tbase | (lane * 4u), lane);
+        DBG_MIN(6); /* first worker warp leaves */
+        DBG_MAX(7); /* last worker warp leaves  */
     }
 }
 

@@ -685,20 +685,32 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     }
     const size_t off_tk = off_key + nkeys * sizeof(aesoff_key_t);
     aesoff_ticket_t *ht = reinterpret_cast<aesoff_ticket_t *>(L.stage + off_tk);
-    uint64_t t = 0;
+    /* The end of a launch is the one place where big units cost: a warp's last row takes 10 us while
+     * the rest of the GPU idles.  The chunks holding the last wave of rows (one row per worker warp)
+     * are therefore cut into 1/8 rows and the four waves before them into half rows.               */
+    uint64_t all_rows = 0;
+    for (size_t i = 0; i < n; ++i) all_rows += rows[i];
+    const uint64_t wave = (uint64_t)sms * AESOFF_WORKER_WARPS;
+    uint64_t t = 0, rows_before = 0;
     for (size_t i = 0; i < n; ++i) {
         hd[i].first_ticket = t;
         for (uint32_t c = 0; c < nch[i]; ++c) {
             aesoff_ticket_t &tk = ht[t + c];
+            const uint64_t left = all_rows - (rows_before + (uint64_t)c * crows[i]); /* rows from this chunk on */
+            const uint32_t mode = left <= wave ? AESOFF_FLAG_FINE : left <= 5 * wave ? AESOFF_FLAG_HALF : 0u;
             tk.ring = (uint32_t)i;
-            tk.chunk = c;
+            tk.chunk = c | (mode << AESOFF_TICKET_MODE_SHIFT);
             tk.keyloc = hd[i].keyloc;
             tk.tag = (uint32_t)(t + c) + 1u;
         }
         t += nch[i];
+        rows_before += rows[i];
     }
     memset(hc, 0, AESOFF_CNT_WORDS * 8);
     hc[AESOFF_CNT_PUBLISHED] = total;
+#ifdef AESOFF_DEBUG
+    hc[20] = hc[23] = hc[26] = ~0ull; /* the atomicMin stamps */
+#endif
     const size_t used = off_tk + (size_t)total * sizeof(aesoff_ticket_t);
 
     bool ok = cudaMemcpyAsync(L.blob, L.stage, used, cudaMemcpyHostToDevice, stream) == cudaSuccess;
@@ -734,6 +746,16 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     g_kernel_launches.fetch_add(1);
     return AES_OK;
 }
+
+#ifdef AESOFF_DEBUG
+/* time stamps of the last launch (globaltimer ns): see DBG_MIN / DBG_MAX in aesoff_kernels.cu */
+extern "C" __attribute__((visibility("default"))) int aesoff_debug_stamps(uint64_t out[8])
+{
+    LaunchCtx &L = g_lc;
+    cudaDeviceSynchronize();
+    return cudaMemcpy(out, L.blob + 20 * 8, 64, cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -1;
+}
+#endif
 
 /* ============================================================================================ */
 /* closed-loop executor (PAPER.md:127-135 worker loop; "50 concurrent clients")      */

@@ -103,9 +103,12 @@ typedef struct __attribute__((aligned(16))) aesoff_key {
     uint32_t pad[4];
 } aesoff_key_t;            /* 256 bytes */
 
+#define AESOFF_TICKET_CHUNK_MASK 0x0fffffffu
+#define AESOFF_TICKET_MODE_SHIFT 28u
 typedef struct __attribute__((aligned(16))) aesoff_ticket {
     uint32_t ring;         /* index of the request in dq / mailbox                                     */
-    uint32_t chunk;
+    uint32_t chunk;        /* bits 0..27 chunk index; bits 28..29 unit size of this chunk:
+                              0 rows, AESOFF_FLAG_FINE 1/8 rows, AESOFF_FLAG_HALF half rows            */
     uint32_t keyloc;
     uint32_t tag;          /* (uint32_t)ticket number + 1; the ring is zeroed at engine start          */
 } aesoff_ticket_t;         /* 16 bytes, written and read as one 128-bit access                         */
