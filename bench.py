@@ -453,9 +453,9 @@ def run_sweep(args):
                     nbuf = max(1, min(total // size, max(depth, 64)))
                     if nbuf < depth:
                         continue  # 64 MiB x 256 and up do not fit 8 GiB: cell skipped, stated in the output
-                    n = max(4 * depth, 64)
-                    while n * size < (256 << 20) and n < 200000:
-                        n *= 2
+                    # about 50 ms of work per cell, from a rough rate estimate
+                    rate = min(600e9 / size, 4e6, depth / 10e-6)
+                    n = int(min(max(0.05 * rate, 4 * depth, 64), 400000))
                     ptrs = np.asarray([buf.data_ptr() + (i % nbuf) * size for i in range(n)], dtype=np.uint64)
                     icb = np.zeros((n, 16), dtype=np.uint8)
                     icb[:, :8] = rng.integers(0, 256, size=(n, 8), dtype=np.uint8)
