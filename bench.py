@@ -47,7 +47,7 @@ UNIT = "GB/s"
 
 # shared-memory lookups per 16-byte block in the CUDA path: per block
 # 1 (round 1) + 4 (round 2) + 16 * (Nr - 2) ; plus 27 per 8 blocks for the per-row constants
-LOOKUPS = {128: 1 + 4 + 16 * 8 + 27 / 8.0, 256: 1 + 4 + 16 * 12 + 27 / 8.0}
+LOOKUPS = {128: 1 + 4 + 16 * 8 + 27 / 8.0, 192: 1 + 4 + 16 * 10 + 27 / 8.0, 256: 1 + 4 + 16 * 12 + 27 / 8.0}
 SMEM_BYTES_PER_CLK_PER_SM = 128.0  # 32 banks x 4 B (guides/B300_MICROARCH.md "smem crossbar BW")
 
 

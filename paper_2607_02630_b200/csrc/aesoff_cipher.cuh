@@ -116,7 +116,7 @@ __device__ __forceinline__ uint32_t sub_word(uint32_t w, uint32_t ybase)
 }
 /* key: Nk little-endian-loaded words of the cipher key; out: 4 (Nk + 7) words in global memory.
  * Words are little-endian loads of the FIPS-197 byte string, so RotWord is a right rotation by 8
- * and Rcon lands in the low byte.  One thread, one serial chain of Nk + 6 (Nk = 4) or 2 x 7 - 1
+ * and Rcon lands in the low byte.  One thread, one serial chain of 10 (Nk = 4), 8 (Nk = 6) or 13
  * (Nk = 8) SubWords: well under a microsecond, against a PCIe round trip for shipping 240 bytes. */
 template <int NK>
 __device__ __noinline__ void key_expand(uint32_t ybase, const uint32_t *key, uint32_t *out)

@@ -594,6 +594,8 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             for (int i = 0; i < 8; ++i) key[i] = PW(AESOFF_PW_RAWKEY + i);
             if (nr == 10)
                 key_expand<4>(ybase, key, P.ktab[keyloc].rk); /* step a1 on the device */
+            else if (nr == 12)
+                key_expand<6>(ybase, key, P.ktab[keyloc].rk);
             else
                 key_expand<8>(ybase, key, P.ktab[keyloc].rk);
         }

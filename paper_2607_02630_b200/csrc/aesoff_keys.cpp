@@ -72,7 +72,7 @@ int aesoff_key_expand(const uint8_t *key, int keybits, uint32_t rk[60])
 {
     std::call_once(g_once, build_tables);
     const int nk = keybits / 32;
-    if (nk != 4 && nk != 8) return -1;
+    if (nk != 4 && nk != 6 && nk != 8) return -1;
     const int nr = nk + 6;
     const int nwords = 4 * (nr + 1);
     for (int i = 0; i < nk; ++i)

@@ -179,7 +179,7 @@ extern "C" const char *aes_strerror(int code)
     switch (code) {
     case AES_OK: return "ok";
     case AES_E_INVAL: return "invalid argument";
-    case AES_E_KEYBITS: return "keybits must be 128 or 256";
+    case AES_E_KEYBITS: return "keybits must be 128, 192 or 256";
     case AES_E_ALIGN: return "src/dst must be 16-byte aligned";
     case AES_E_OVERLAP: return "src and dst overlap partially";
     case AES_E_AGAIN: return "submission ring full";
@@ -201,7 +201,7 @@ extern "C" aes_ctx_t *aes_ctx_create(const uint8_t *key, int keybits)
         fail(AES_E_INVAL);
         return nullptr;
     }
-    if (keybits != 128 && keybits != 256) {
+    if (keybits != 128 && keybits != 192 && keybits != 256) {
         fail(AES_E_KEYBITS);
         return nullptr;
     }

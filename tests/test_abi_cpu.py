@@ -49,7 +49,8 @@ def test_no_torch_types_in_abi():
 
 def test_key_expansion_matches_oracle_and_fips_appendix_a(P, golden):
     rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 90]))
-    keys = [rng.bytes(16) for _ in range(50)] + [rng.bytes(32) for _ in range(50)] + [bytes(16), bytes(32), b"\xff" * 32]
+    keys = ([rng.bytes(16) for _ in range(50)] + [rng.bytes(24) for _ in range(50)] + [rng.bytes(32) for _ in range(50)]
+            + [bytes(16), bytes(24), bytes(32), b"\xff" * 32])
     for key in keys:
         ctx = P.aes_ctx_create(key)
         rk, nr = P.aes_ctx_round_keys(ctx)
@@ -62,6 +63,10 @@ def test_key_expansion_matches_oracle_and_fips_appendix_a(P, golden):
     rk, nr = P.aes_ctx_round_keys(ctx)
     P.aes_ctx_destroy(ctx)
     assert nr == 10 and rk[16:32] == g["a1.w4_w7"] and rk[160:176] == g["a1.w40_w43"]
+    ctx = P.aes_ctx_create(g["a2.key"])
+    rk, nr = P.aes_ctx_round_keys(ctx)
+    P.aes_ctx_destroy(ctx)
+    assert nr == 12 and rk[24:28] == g["a2.w6"] and rk[192:208] == g["a2.w48_w51"]
     ctx = P.aes_ctx_create(g["a3.key"])
     rk, nr = P.aes_ctx_round_keys(ctx)
     P.aes_ctx_destroy(ctx)
@@ -70,7 +75,7 @@ def test_key_expansion_matches_oracle_and_fips_appendix_a(P, golden):
 
 def test_ctx_errors(P):
     with pytest.raises(P.AesOffError) as e:
-        P.aes_ctx_create(bytes(24))  # AES-192 is not on the GPU path (north_star: 128 and 256)
+        P.aes_ctx_create(bytes(20))
     assert e.value.code == P.AES_E_KEYBITS
     with pytest.raises(P.AesOffError) as e:
         P.aes_ctx_create(bytes(16), keybits=100)

@@ -86,7 +86,7 @@ def test_config1_single_request(P):
 def test_lengths_and_carries(P):
     rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7000]))
     reqs = []
-    for keylen in (16, 32):
+    for keylen in (16, 24, 32):
         key = rng.bytes(keylen)
         for n in (0, 1, 15, 16, 17, 4095, 4096, 4097, 16385, 65536 + 5, (1 << 20) + 5):
             reqs.append((key, rng.bytes(8) + bytes(8), np.frombuffer(rng.bytes(n), dtype=np.uint8)))
@@ -312,7 +312,7 @@ def test_context_key_paths(P):
     src = G.to_device(data)
     G.stream_sync()
     # (a) one context, six submits: raw, raw+install, four by index; both key sizes
-    for keylen in (16, 32):
+    for keylen in (16, 24, 32):
         key = rng.bytes(keylen)
         ctx = P.aes_ctx_create(key)
         for j in range(6):
@@ -329,7 +329,7 @@ def test_context_key_paths(P):
     dsts = G.device_empty(n_ctx * per * 96)
     keys, icbs, hs = [], [], []
     for i in range(n_ctx):
-        key = rng.bytes(16 if i % 2 else 32)
+        key = rng.bytes((16, 24, 32)[i % 3])
         ctx = P.aes_ctx_create(key)
         for j in range(per):
             icb = rng.bytes(16)

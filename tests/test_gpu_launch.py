@@ -60,7 +60,7 @@ def test_config1_aes128_64KiB(P):
     _check(P, [(w.key_of(0), w.icb_of(0), w.payload(0))])
 
 
-@pytest.mark.parametrize("keylen", [16, 32])
+@pytest.mark.parametrize("keylen", [16, 24, 32])
 def test_lengths_tails_and_tiles(P, keylen):
     """Empty, sub-block, block +-1, row (4 KiB) +-1, chunk (16 KiB) +-1, several chunks + ragged tail."""
     rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 1000 + keylen]))
@@ -74,7 +74,7 @@ def test_lengths_tails_and_tiles(P, keylen):
     _check(P, reqs)
 
 
-@pytest.mark.parametrize("keylen", [16, 32])
+@pytest.mark.parametrize("keylen", [16, 24, 32])
 def test_counter_carries(P, keylen):
     """R4: the counter is a 128-bit big-endian integer; carries out of the low 8/32/64/128 bits, both
     on the first increment and in the middle of a chunk, and ICBs whose last byte is not zero (rows
