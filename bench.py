@@ -204,12 +204,16 @@ def main():
     ap.add_argument("--chunk-rows", type=int, default=0)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e / latency / cpu_baseline / kernel-only legs")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: size x in-flight x key-size table (one GPU)")
-    ap.add_argument("--sweep-out", default="", help="with --sweep: also write the table to this JSON file")
+    ap.add_argument("--sweep-out", default="", help="with --sweep / --openloop: also write the table to this JSON file")
+    ap.add_argument("--openloop", action="store_true", help="latency under Poisson load, blocking vs overlapping (PAPER.md:244)")
+    ap.add_argument("--openloop-bytes", type=int, default=4096)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
     if args.sweep:
         return run_sweep(args)
+    if args.openloop:
+        return run_openloop(args)
     if args.warmup < 3:
         args.warmup = 3
 
@@ -480,6 +484,50 @@ def run_sweep(args):
             json.dump({"lookup_roof_gbs_of_lookup_bytes": lds_peak, "hbm_peak_gbs": hbm_peak, "sm_mhz_assumed": sm_max_mhz,
                        "note": "in place; 64 MiB x 256/1024 in flight skipped (needs more than the 8 GiB the sweep allocates)",
                        "cells": cells}, f, indent=1)
+    return 0
+
+
+def run_openloop(args):
+    """The paper's latency-under-load experiment (Fig. 12) with the REAL offload instead of the
+    paper's 20 us emulated one: Poisson arrivals of 4 KiB AES-128-CTR requests at a swept offered load, one
+    server thread that either waits for each offload (blocking) or keeps serving and polls (overlapping)."""
+    import torch
+
+    import paper_2607_02630_b200.binding as B
+
+    dev = torch.device("cuda", 0)
+    size, pool = args.openloop_bytes, 4096
+    buf = torch.empty(2 * pool * size, dtype=torch.uint8, device=dev)
+    buf.random_(0, 256)
+    torch.cuda.synchronize()
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE + 6, 1]))
+    ctx = B.aes_ctx_create(rng.bytes(16))
+    rows = []
+    B.aes_engine_start(0, idle_exit_ms=30000)
+    try:
+        for rate in (25e3, 50e3, 75e3, 100e3, 150e3, 200e3, 400e3, 800e3, 1.6e6, 2.4e6, 3.2e6, 4.0e6, 4.8e6):
+            n = int(min(max(rate * 0.05, 2000), 200000))
+            gaps = rng.exponential(1e9 / rate, size=n)
+            arrival = np.cumsum(gaps).astype(np.uint64)
+            icb = rng.integers(0, 256, size=(n, 16), dtype=np.uint8)
+            srcs = np.asarray([buf.data_ptr() + (i % pool) * size for i in range(n)], dtype=np.uint64)
+            dsts = np.asarray([buf.data_ptr() + (pool + i % pool) * size for i in range(n)], dtype=np.uint64)
+            lens = np.full(n, size, dtype=np.uint64)
+            row = {"offered_req_per_s": rate, "bytes": size, "requests": n}
+            for mode in ("overlapping", "blocking"):
+                r = B.aes_openloop_run(icb, srcs, dsts, lens, arrival, ctx, blocking=(mode == "blocking"))
+                a = r["lat_ns"][n // 20:] / 1e3
+                row[mode] = {"p50_us": percentile(a, 50), "p99_us": percentile(a, 99),
+                             "achieved_req_per_s": n / (r["elapsed_ns"] * 1e-9), "max_in_flight": int(r["max_in_flight"]),
+                             "ring_full": int(r["ring_full_spins"])}
+            rows.append(row)
+            print(json.dumps(row), flush=True)
+    finally:
+        B.aes_engine_stop()
+        B.aes_ctx_destroy(ctx)
+    if args.sweep_out:
+        with open(args.sweep_out, "w") as f:
+            json.dump({"rows": rows}, f, indent=1)
     return 0
 
 

@@ -222,6 +222,17 @@ typedef struct aes_loop_result {
 /* Returns AES_OK or the first error.  lat_ns: host, n*repeat doubles or NULL.      */
 int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res, double *lat_ns);
 
+/* ---- open-loop executor (the paper's latency-under-load experiment, Fig. 12) ----
+ * Request i arrives arrival_ns[i] nanoseconds after the call starts (host array of spec->n
+ * non-decreasing offsets; the caller draws them, e.g. Poisson) and is submitted as soon as that
+ * time has passed, whatever is still in flight.  blocking == 0: the loop goes on serving arrivals
+ * and polls completions in between (the rerouted server); blocking != 0: it waits for each offload
+ * before it looks at the next arrival (the server the paper starts from).  lat_ns[i] = completion
+ * observed - arrival time, so queueing in front of a busy loop counts.  spec->ctx is required
+ * (keys, window and repeat are ignored).  Returns AES_OK or the first error.                     */
+int aes_openloop_run(const aes_loop_spec_t *spec, const uint64_t *arrival_ns, int blocking,
+                     aes_loop_result_t *res, double *lat_ns);
+
 #if defined(__GNUC__)
 #pragma GCC visibility pop
 #endif

@@ -88,6 +88,7 @@ def _load() -> ctypes.CDLL:
         "aes_host_alloc": (vp, [sz]),
         "aes_host_free": (None, [vp]),
         "aes_loop_run": (i32, [vp, vp, vp]),
+        "aes_openloop_run": (i32, [vp, vp, i32, vp, vp]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(L, name)
@@ -99,7 +100,7 @@ def _load() -> ctypes.CDLL:
 _lib = _load()
 EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_ctx_create", "aes_ctx_destroy",
            "aes_ctx_round_keys", "aes_ctr_submit", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
-           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run")
+           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run", "aes_openloop_run")
 
 
 def aes_strerror(code: int) -> str:
@@ -232,6 +233,27 @@ def aes_loop_run(nonces, srcs, dsts, lens, window: int, ctx: int = 0, keys=None,
     lat = np.zeros(n * repeat, dtype=np.float64) if want_latency else None
     _check(_lib.aes_loop_run(ctypes.byref(spec), ctypes.byref(res), lat.ctypes.data if lat is not None else None),
            "aes_loop_run")
+    out = {k: getattr(res, k) for k, _ in aes_loop_result_t._fields_}
+    out["lat_ns"] = lat
+    return out
+
+
+def aes_openloop_run(nonces, srcs, dsts, lens, arrival_ns, ctx: int, blocking: bool = False) -> dict:
+    """Runs the native open loop (see aes_openloop_run in aesoff.h): request i is submitted once
+    arrival_ns[i] has passed.  Returns elapsed_ns, bytes, requests, ring_full_spins, max_in_flight, lat_ns."""
+    n = len(lens)
+    a_src, a_dst, a_len = _ptr_array(srcs), _ptr_array(dsts), _ptr_array(lens)
+    a_non = np.ascontiguousarray(np.asarray(nonces, dtype=np.uint8)).reshape(-1)
+    a_arr = np.ascontiguousarray(np.asarray(arrival_ns, dtype=np.uint64))
+    assert a_non.size == 16 * n and a_arr.size == n
+    spec = aes_loop_spec_t()
+    spec.n, spec.window, spec.repeat = n, 0, 1
+    spec.ctx = ctx
+    spec.nonces, spec.srcs, spec.dsts, spec.lens = a_non.ctypes.data, a_src.ctypes.data, a_dst.ctypes.data, a_len.ctypes.data
+    res = aes_loop_result_t()
+    lat = np.zeros(n, dtype=np.float64)
+    _check(_lib.aes_openloop_run(ctypes.byref(spec), a_arr.ctypes.data, 1 if blocking else 0, ctypes.byref(res),
+                                 lat.ctypes.data), "aes_openloop_run")
     out = {k: getattr(res, k) for k, _ in aes_loop_result_t._fields_}
     out["lat_ns"] = lat
     return out

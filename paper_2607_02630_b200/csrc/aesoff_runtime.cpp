@@ -827,3 +827,74 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
     res->requests = done;
     return AES_OK;
 }
+
+/* ============================================================================================ */
+/* open-loop executor (Fig. 12: Poisson arrivals, blocking vs overlapping)          */
+/* ============================================================================================ */
+extern "C" int aes_openloop_run(const aes_loop_spec_t *spec, const uint64_t *arrival_ns, int blocking,
+                                aes_loop_result_t *res, double *lat_ns)
+{
+    if (!spec || !res || !arrival_ns || !spec->ctx || !spec->nonces || !spec->srcs || !spec->dsts || !spec->lens)
+        return fail(AES_E_INVAL);
+    if (spec->n == 0) return fail(AES_E_INVAL);
+    Engine &e = g_eng;
+    if (e.running.load() != 1) return fail(AES_E_STOPPED);
+    const size_t n = spec->n;
+    struct Fly {
+        aes_handle_t h;
+        size_t index;
+    };
+    std::vector<Fly> fly;
+    fly.reserve(e.R);
+    memset(res, 0, sizeof(*res));
+    size_t next = 0, done = 0;
+    uint64_t bytes = 0;
+    const uint64_t t0 = now_ns();
+    while (done < n) {
+        uint64_t now = now_ns() - t0;
+        /* every request whose arrival time has passed is submitted (the ring bounds what is in flight) */
+        while (next < n && arrival_ns[next] <= now) {
+            const aes_handle_t h = aes_ctr_submit(spec->ctx, spec->nonces + 16 * next, spec->srcs[next], spec->dsts[next],
+                                                  spec->lens[next]);
+            if (h == 0) {
+                if (t_last_error == AES_E_AGAIN) {
+                    ++res->ring_full_spins;
+                    break;
+                }
+                return t_last_error;
+            }
+            if (blocking) {
+                /* the server that waits for its offload: nothing else is served meanwhile */
+                const int rc = aes_wait(h, UINT64_MAX);
+                if (rc != AES_OK) return rc;
+                now = now_ns() - t0;
+                if (lat_ns) lat_ns[next] = (double)(now - arrival_ns[next]);
+                bytes += spec->lens[next];
+                ++done;
+            } else {
+                fly.push_back(Fly{h, next});
+                if (fly.size() > res->max_in_flight) res->max_in_flight = fly.size();
+            }
+            ++next;
+        }
+        size_t k = 0;
+        while (k < fly.size()) {
+            const int r = aes_poll(fly[k].h);
+            if (r == 1) {
+                if (lat_ns) lat_ns[fly[k].index] = (double)(now_ns() - t0 - arrival_ns[fly[k].index]);
+                bytes += spec->lens[fly[k].index];
+                ++done;
+                fly[k] = fly.back();
+                fly.pop_back();
+            } else if (r < 0) {
+                return r;
+            } else {
+                ++k;
+            }
+        }
+    }
+    res->elapsed_ns = now_ns() - t0;
+    res->bytes = bytes;
+    res->requests = done;
+    return AES_OK;
+}
