@@ -21,7 +21,7 @@ def torch_cuda():
 def to_device(arr: np.ndarray):
     """uint8 numpy -> uint8 CUDA tensor (16-byte aligned by the caching allocator)."""
     torch = torch_cuda()
-    t = torch.from_numpy(np.ascontiguousarray(arr)).to("cuda:0", non_blocking=False)
+    t = torch.from_numpy(np.array(arr)).to("cuda:0", non_blocking=False)  # a writable copy
     assert t.data_ptr() % 16 == 0
     return t
 
