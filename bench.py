@@ -608,6 +608,17 @@ def extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, s
     B.aes_host_free(hs)
     B.aes_host_free(hd)
 
+    # ---- calibration: what the lookup pipe, the ALU pipe and the payload path deliver on this GPU ----
+    try:
+        cal = B.aes_calibrate(local_rank)
+        cal["lookup_pipe_frac_of_nominal"] = cal["lookups_per_clk_per_sm"] / 32.0
+        cal["main_round_frac_of_nominal"] = cal["round_lookups_per_clk_per_sm"] / 32.0
+        cal["how"] = ("aes_calibrate: microkernels with the engine's table layout and launch shape; nominal = 32 lookups and "
+                      "2 warp-wide ALU instructions per clock per SM (guides/B300_MICROARCH.md)")
+        res["calibration"] = cal
+    except Exception as e:  # noqa: BLE001
+        res["calibration"] = {"error": str(e)}
+
     # ---- cpu_baseline: the oracle, as it stands, on the host cores, bounded sample ----
     cores = len(os.sched_getaffinity(0))
     n_cpu = min(n, 16 * cores)

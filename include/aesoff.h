@@ -222,6 +222,26 @@ typedef struct aes_loop_result {
 /* Returns AES_OK or the first error.  lat_ns: host, n*repeat doubles or NULL.      */
 int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res, double *lat_ns);
 
+/* ---- calibration ---------------------------
+ * Runs three microkernels with the engine's own table layout and launch shape and reports what the
+ * units the cipher leans on deliver on this GPU: table lookups (PRMT + conflict-free LDS.32) per
+ * clock per SM, warp-wide ALU instructions (PRMT / LOP3) per clock per SM, the lookup rate of the
+ * cipher's main round as it stands, and the GB/s (read + write) of 128-bit L2-only loads and
+ * stores over 2 x 1 GiB.  Not on the product path: bench.py and
+ * the tests call it.  The engine must not be running (AES_E_BUSY).  Returns AES_OK / AES_E_CUDA.   */
+typedef struct aes_calib {
+    double  lookups_per_clk_per_sm;      /* nominal 32 (128 B/clk/SM)                         */
+    double  alu_instr_per_clk_per_sm;    /* warp-wide; nominal 2 (64 lanes/clk/SM)            */
+    double  copy_gbs;
+    double  sm_mhz;                      /* SM clock seen by the lookup run                   */
+    int32_t sm_count;
+    int32_t reserved;
+    double  round_lookups_per_clk_per_sm; /* lookups per clock per SM of the cipher's own main
+                                             round (4 PRMT + 4 LDS + 2 LOP3 per column): what the
+                                             two pipes deliver together                        */
+} aes_calib_t;
+int aes_calibrate(int device, aes_calib_t *out);
+
 /* ---- open-loop executor (the paper's latency-under-load experiment, Fig. 12) ----
  * Request i arrives arrival_ns[i] nanoseconds after the call starts (host array of spec->n
  * non-decreasing offsets; the caller draws them, e.g. Poisson) and is submitted as soon as that

@@ -53,6 +53,12 @@ class aes_engine_info_t(ctypes.Structure):
                 ("cut_eighths", ctypes.c_uint64), ("cut_halves", ctypes.c_uint64), ("cut_rows", ctypes.c_uint64)]
 
 
+class aes_calib_t(ctypes.Structure):
+    _fields_ = [("lookups_per_clk_per_sm", ctypes.c_double), ("alu_instr_per_clk_per_sm", ctypes.c_double),
+                ("copy_gbs", ctypes.c_double), ("sm_mhz", ctypes.c_double), ("sm_count", ctypes.c_int32),
+                ("reserved", ctypes.c_int32), ("round_lookups_per_clk_per_sm", ctypes.c_double)]
+
+
 class aes_loop_spec_t(ctypes.Structure):
     _fields_ = [("n", ctypes.c_size_t), ("window", ctypes.c_uint32), ("repeat", ctypes.c_uint32),
                 ("ctx", ctypes.c_void_p), ("keys", ctypes.c_void_p), ("keybits", ctypes.c_void_p),
@@ -89,6 +95,7 @@ def _load() -> ctypes.CDLL:
         "aes_host_free": (None, [vp]),
         "aes_loop_run": (i32, [vp, vp, vp]),
         "aes_openloop_run": (i32, [vp, vp, i32, vp, vp]),
+        "aes_calibrate": (i32, [i32, vp]),
     }
     for name, (res, args) in sigs.items():
         fn = getattr(L, name)
@@ -100,7 +107,7 @@ def _load() -> ctypes.CDLL:
 _lib = _load()
 EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_ctx_create", "aes_ctx_destroy",
            "aes_ctx_round_keys", "aes_ctr_submit", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
-           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run", "aes_openloop_run")
+           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run", "aes_openloop_run", "aes_calibrate")
 
 
 def aes_strerror(code: int) -> str:
@@ -257,3 +264,10 @@ def aes_openloop_run(nonces, srcs, dsts, lens, arrival_ns, ctx: int, blocking: b
     out = {k: getattr(res, k) for k, _ in aes_loop_result_t._fields_}
     out["lat_ns"] = lat
     return out
+
+
+def aes_calibrate(device: int = 0) -> dict:
+    """Calibration microkernels (see aes_calibrate in aesoff.h)."""
+    c = aes_calib_t()
+    _check(_lib.aes_calibrate(device, ctypes.byref(c)), "aes_calibrate")
+    return {k: getattr(c, k) for k, _ in aes_calib_t._fields_ if k != "reserved"}

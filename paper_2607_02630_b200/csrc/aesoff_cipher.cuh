@@ -63,7 +63,7 @@ __device__ __forceinline__ uint32_t rotl32(uint32_t x, int n) { return __funnels
 __device__ __forceinline__ uint32_t bitsel(uint32_t a, uint32_t b, uint32_t m) { return (a & m) | (b & ~m); }
 
 /* at most one block per request takes this path, so it is kept out of line */
-__device__ __noinline__ void store_partial(const uint8_t *src, uint8_t *dst, uint32_t o0, uint32_t o1, uint32_t o2,
+static __device__ __noinline__ void store_partial(const uint8_t *src, uint8_t *dst, uint32_t o0, uint32_t o1, uint32_t o2,
                                            uint32_t o3, uint32_t u)
 {
 #pragma unroll 1

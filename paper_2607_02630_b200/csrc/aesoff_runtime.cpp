@@ -829,6 +829,27 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
 }
 
 /* ============================================================================================ */
+/* calibration microkernels (aesoff_calib.cu)                                                     */
+/* ============================================================================================ */
+extern "C" int aes_calibrate(int device, aes_calib_t *out)
+{
+    if (!out) return fail(AES_E_INVAL);
+    if (g_eng.running.load()) return fail(AES_E_BUSY);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(AES_E_CUDA);
+    double v[6];
+    if (aesoff_run_calibration(device, v) != 0) return fail(AES_E_CUDA);
+    out->lookups_per_clk_per_sm = v[0] * 32.0; /* the kernel counts warp-wide LDS instructions */
+    out->alu_instr_per_clk_per_sm = v[1];
+    out->copy_gbs = v[2];
+    out->sm_mhz = v[3];
+    out->sm_count = (int32_t)v[4];
+    out->reserved = 0;
+    out->round_lookups_per_clk_per_sm = v[5] * 32.0;
+    return AES_OK;
+}
+
+/* ============================================================================================ */
 /* open-loop executor (Fig. 12: Poisson arrivals, blocking vs overlapping)          */
 /* ============================================================================================ */
 extern "C" int aes_openloop_run(const aes_loop_spec_t *spec, const uint64_t *arrival_ns, int blocking,

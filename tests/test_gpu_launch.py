@@ -161,3 +161,15 @@ def test_errors_launch(P):
         P.aes_ctr_launch_batch([0], bytes(16), [p], [p], [64])
     assert e.value.code == P.AES_E_INVAL
     P.aes_ctx_destroy(ctx)
+
+
+def test_calibration_microkernels(P):
+    """aes_calibrate: the lookup pipe delivers (nearly) its nominal 32 lookups per clock per SM with the engine's
+    table layout -- i.e. the layout is conflict-free in fact, not only by construction -- and the ALU pipe its
+    nominal 2 warp-wide instructions; the numbers bench.py's roofline stands on."""
+    c = P.aes_calibrate(0)
+    assert c["sm_count"] >= 100
+    assert 28.0 <= c["lookups_per_clk_per_sm"] <= 32.5, c
+    assert 26.0 <= c["round_lookups_per_clk_per_sm"] <= 32.5, c
+    assert 1.7 <= c["alu_instr_per_clk_per_sm"] <= 2.1, c
+    assert c["copy_gbs"] > 3000.0, c
