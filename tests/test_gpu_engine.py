@@ -372,7 +372,9 @@ def test_unit_sizes_half_rows_and_eighths(P):
     d = {k: after[k] - before[k] for k in ("cut_eighths", "cut_halves", "cut_rows")}
     assert sum(d.values()) == len(lone) + len(short) + len(long_q)
     if P.test_latency_units:
-        assert d["cut_eighths"] >= 1 and d["cut_halves"] >= 1 and d["cut_rows"] >= 1, d
+        # which size a request gets depends on the load it meets, i.e. on timing: the lone request finds the GPU
+        # idle (1/8 rows); most of the 48 x 2 MiB queue must have been cut coarser than that
+        assert d["cut_eighths"] >= 1 and d["cut_halves"] + d["cut_rows"] >= len(long_q) // 2, d
     else:
         assert d["cut_rows"] == sum(d.values())
 
