@@ -48,6 +48,16 @@ UNIT = "GB/s"
 # shared-memory lookups per 16-byte block in the CUDA path: per block
 # 1 (round 1) + 4 (round 2) + 16 * (Nr - 2) ; plus 27 per 8 blocks for the per-row constants
 LOOKUPS = {128: 1 + 4 + 16 * 8 + 27 / 8.0, 192: 1 + 4 + 16 * 10 + 27 / 8.0, 256: 1 + 4 + 16 * 12 + 27 / 8.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the launch backend, from the ncu --set full captures
+# summarised in profiles/r1c_ncu.md (a persistent launch cannot be replayed by ncu)
+NCU_TRAFFIC = {
+    "c2": {"bytes": 67.25e6 + 25.27e6,
+           "how": "ncu, one 64 x 1 MiB launch of the launch backend: 67.25 MB read + 25.27 MB written (algorithmic 67.11 + "
+                  "67.11; the rest of the writes is still in the 126 MB L2 when the kernel ends); profiles/r1c_ncu.md"},
+    "c3": {"bytes": 134.42e6 + 93.36e6,
+           "how": "ncu, one 16 x 8 MiB launch of the launch backend: 134.42 MB read + 93.36 MB written (algorithmic 134.22 + "
+                  "134.22); profiles/r1c_ncu.md"},
+}
 SMEM_BYTES_PER_CLK_PER_SM = 128.0  # 32 banks x 4 B (guides/B300_MICROARCH.md "smem crossbar BW")
 
 
@@ -376,7 +386,8 @@ def main():
         "lookups_per_block": LOOKUPS[keybits], "payload_gbs": kern_payload_gbs,
         "hbm": {"achieved": 2 * kern_payload_gbs, "peak": hbm_peak, "unit": "GB/s",
                 "frac": 2 * kern_payload_gbs / hbm_peak, "peak_kind": peak_kind},
-        "traffic": None, "avg_launch_ms": kernel_ms, "how": how,
+        "traffic": NCU_TRAFFIC.get(args.workload, {}).get("bytes"), "traffic_how": NCU_TRAFFIC.get(args.workload, {}).get("how"),
+        "avg_launch_ms": kernel_ms, "how": how,
     }
 
     out = {
@@ -626,7 +637,30 @@ def extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, s
     res["cpu_baseline"] = {"value": gbs, "unit": UNIT, "cores": cores, "kind": "oracle",
                            "sample": "first %d of %d requests of %s (%d MiB), one thread per core, %.1f s" % (
                                n_cpu, n, w.name, n_cpu * size // MIB, dt)}
+    res["cpu_context_aesni"] = openssl_speed(keybits)
     return res
+
+
+def openssl_speed(keybits):
+    """Second context line: OpenSSL's AES-NI/VAES CTR on ONE host core, because the paper
+    itself notes that 'a modern core's AES-NI rivals a GPU on this cipher'.  Not a target."""
+    import re
+    import shutil
+    import subprocess
+
+    exe = shutil.which("openssl")
+    if not exe:
+        return {"unavailable": "no openssl binary on this box"}
+    try:
+        out = subprocess.run([exe, "speed", "-elapsed", "-evp", "aes-%d-ctr" % keybits, "-bytes", "1048576", "-seconds", "1"],
+                             capture_output=True, text=True, timeout=30).stdout
+        m = re.search(r"^AES-%d-CTR\s+([0-9.]+)k" % keybits, out, re.M | re.I)
+        if not m:
+            return {"unavailable": "could not parse openssl speed output"}
+        return {"value": float(m.group(1)) * 1000.0 / 1e9, "unit": UNIT, "cores": 1,
+                "kind": "openssl speed -evp aes-%d-ctr, 1 MiB blocks (AES-NI/VAES)" % keybits}
+    except Exception as e:  # noqa: BLE001
+        return {"unavailable": str(e)}
 
 
 if __name__ == "__main__":
