@@ -46,9 +46,11 @@ struct __align__(16) Slot {
     uint32_t unit0_row;     /* first row of this chunk                                          */
     uint32_t ring_slot;     /* index of the request in dq / mailbox                             */
     uint32_t n_units;
-    uint32_t fine;          /* unit size: 0 a row, AESOFF_FLAG_HALF half a row (128 blocks),
+    uint32_t n_rows;        /* rows of this chunk                                               */
+    uint32_t pad_[3];
+    uint32_t fine;          /* unit size: 0 rows (AESOFF_ROWS_PER_UNIT of them), AESOFF_FLAG_HALF half a row (128 blocks),
                                AESOFF_FLAG_FINE one k-iteration of a row (32 blocks)            */
-};                          /* 368 B */
+};                          /* 384 B */
 
 struct __align__(16) CtaCtl {
     Slot slot[AESOFF_SLOTS];
@@ -201,8 +203,14 @@ __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase,
             const uint64_t m = (uint64_t)sl->unit0_row + (u >> 1);
             ctr_request_row<4>(ybase, rk4, nr, g, src, dst, len, m, lane, (u & 1u) * 4u, (u & 1u) * 4u + 4u);
         } else {
-            const uint64_t m = (uint64_t)sl->unit0_row + u;
-            ctr_request_row<AESOFF_NB>(ybase, rk4, nr, g, src, dst, len, m, lane);
+            /* a whole-row unit is AESOFF_ROWS_PER_UNIT consecutive rows: half the claims and done counts */
+            const uint32_t crows_here = sl->n_rows;
+#pragma unroll 1
+            for (uint32_t rr = 0; rr < AESOFF_ROWS_PER_UNIT; ++rr) {
+                const uint32_t ri = u * AESOFF_ROWS_PER_UNIT + rr;
+                if (ri >= crows_here) break;
+                ctr_request_row<AESOFF_NB>(ybase, rk4, nr, g, src, dst, len, (uint64_t)sl->unit0_row + ri, lane);
+            }
         }
         __syncwarp();
         if (lane == 0) {
@@ -273,7 +281,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
                 const uint32_t w = lds_volatile(&c->claim[lane]);
                 const uint32_t left = (w >> 16) > (w & 0xffffu) ? (w >> 16) - (w & 0xffffu) : 0u;
                 const uint32_t f = c->slot[lane].fine;
-                held = (f & AESOFF_FLAG_FINE) ? left : (f & AESOFF_FLAG_HALF) ? left * 4u : left * 8u;
+                held = (f & AESOFF_FLAG_FINE) ? left : (f & AESOFF_FLAG_HALF) ? left * 4u : left * 8u * AESOFF_ROWS_PER_UNIT;
             } else if (have) {
                 held = per_ticket;
             }
@@ -352,7 +360,9 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
                 const unsigned long long row0 = (unsigned long long)chunk * crows;
                 const uint32_t nrows = (uint32_t)((rows - row0) < crows ? (rows - row0) : crows);
                 const uint32_t fine = unit_mode & (AESOFF_FLAG_FINE | AESOFF_FLAG_HALF);
-                const uint32_t n_units = (fine & AESOFF_FLAG_FINE) ? nrows * 8u : (fine & AESOFF_FLAG_HALF) ? nrows * 2u : nrows;
+                const uint32_t n_units = (fine & AESOFF_FLAG_FINE) ? nrows * 8u : (fine & AESOFF_FLAG_HALF) ? nrows * 2u
+                                         : (nrows + AESOFF_ROWS_PER_UNIT - 1u) / AESOFF_ROWS_PER_UNIT;
+                sl->n_rows = nrows;
                 sl->unit0_row = (uint32_t)row0;
                 sl->ring_slot = ring;
                 sl->n_units = n_units;

@@ -26,6 +26,7 @@
 #ifndef AESOFF_WORKER_WARPS
 #define AESOFF_WORKER_WARPS    16u    /* warps that run the cipher; 4 per SM sub-partition               */
 #endif
+#define AESOFF_ROWS_PER_UNIT   2u     /* whole-row units (saturation) are this many consecutive rows      */
 #ifndef AESOFF_NB
 #define AESOFF_NB              4      /* blocks a lane keeps in flight through the rounds (row units)     */
 #endif
