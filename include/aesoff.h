@@ -86,7 +86,11 @@ typedef struct aes_engine_opts {
  * Returns AES_OK, AES_E_BUSY if already running, AES_E_INVAL, AES_E_CUDA, AES_E_NOMEM.
  * While the engine runs, a device-wide synchronisation (cudaDeviceSynchronize,
  * cudaFree, torch.cuda.synchronize) blocks until aes_engine_stop(): synchronise
- * on streams or events instead.                                                  */
+ * on streams or events instead.  Copies and other kernels run beside the engine
+ * (it leaves 1,472 threads and 10 K registers per SM), with one catch: the FIRST
+ * launch of a kernel whose module CUDA has not loaded yet (lazy loading) blocks
+ * until the engine stops -- launch every kernel once before aes_engine_start, or
+ * run with CUDA_MODULE_LOADING=EAGER.                                              */
 int aes_engine_start(int device, const aes_engine_opts_t *opts);
 
 /* Waits for every accepted request to complete, makes the persistent kernel exit,

@@ -32,3 +32,105 @@ def test_installed_context_survives_restart():
         finally:
             B.aes_engine_stop()
     B.aes_ctx_destroy(ctx)
+
+
+def test_idle_exit_is_detected_and_engine_restarts():
+    """Failure detection: a persistent kernel that has exited -- here by its own idle
+    timer -- is seen through the host-mapped alive word: submits fail with AES_E_STOPPED instead of hanging,
+    aes_engine_stop still returns, and a fresh start serves requests again."""
+    import time
+
+    import gpu_util as G
+    import paper_2607_02630_b200.binding as B
+    from oracle import oracle as o
+
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7710]))
+    key, icb = rng.bytes(16), rng.bytes(16)
+    data = np.frombuffer(rng.bytes(5000), dtype=np.uint8)
+    src, dst = G.to_device(data), G.device_empty(len(data))
+    G.stream_sync()
+    ctx = B.aes_ctx_create(key)
+    B.aes_engine_start(0, idle_exit_ms=50)
+    try:
+        B.aes_wait(B.aes_ctr_submit(ctx, icb, src.data_ptr(), dst.data_ptr(), len(data)))
+        assert B.aes_engine_info()["running"] == 1
+        deadline = time.time() + 5.0
+        while B.aes_engine_info()["running"] == 1 and time.time() < deadline:
+            time.sleep(0.02)
+        assert B.aes_engine_info()["running"] == 0, "the kernel should have left after 50 ms without requests"
+        with pytest.raises(B.AesOffError) as e:
+            B.aes_ctr_submit(ctx, icb, src.data_ptr(), dst.data_ptr(), len(data))
+        assert e.value.code == B.AES_E_STOPPED
+    finally:
+        B.aes_engine_stop()
+    B.aes_engine_start(0, idle_exit_ms=60000)
+    try:
+        dst = G.to_device(np.zeros(len(data), dtype=np.uint8))  # a copy, not a kernel: the engine owns the SMs
+        G.stream_sync()
+        B.aes_wait(B.aes_ctr_submit(ctx, icb, src.data_ptr(), dst.data_ptr(), len(data)))
+        assert dst.cpu().numpy().tobytes() == o.ctr(key, icb, data)
+    finally:
+        B.aes_engine_stop()
+    B.aes_ctx_destroy(ctx)
+
+
+def test_wait_timeout_then_completion():
+    """aes_wait with a 1 ns budget on a 256 MiB request times out (AES_E_TIMEOUT) without disturbing the request;
+    a later wait sees it complete, bit-exact on sampled windows."""
+    import gpu_util as G
+    import paper_2607_02630_b200.binding as B
+    from oracle import oracle as o
+
+    torch = G.torch_cuda()
+    n = 256 << 20
+    big = torch.zeros(n, dtype=torch.uint8, device="cuda:0")
+    out = torch.empty_like(big)
+    torch.cuda.synchronize()
+    key, icb = bytes(range(32)), bytes(range(16))
+    ctx = B.aes_ctx_create(key)
+    B.aes_engine_start(0, idle_exit_ms=60000)
+    try:
+        h = B.aes_ctr_submit(ctx, icb, big.data_ptr(), out.data_ptr(), n)
+        with pytest.raises(B.AesOffError) as e:
+            B.aes_wait(h, 1)
+        assert e.value.code == B.AES_E_TIMEOUT
+        B.aes_wait(h, 20_000_000_000)
+        assert B.aes_poll(h) is True
+        zeros = np.zeros(4096, dtype=np.uint8)
+        for off in (0, 4096 * 12345, n - 4096):
+            assert out[off:off + 4096].cpu().numpy().tobytes() == o.ctr(key, icb, zeros, off // 16)
+    finally:
+        B.aes_engine_stop()
+    B.aes_ctx_destroy(ctx)
+
+
+def test_other_kernels_run_beside_the_engine():
+    """A kernel of the process's own (a torch fill, launched once before so that CUDA has its module loaded)
+    completes while the full-size engine is running, and the engine still computes bit-exact."""
+    import time
+
+    import gpu_util as G
+    import paper_2607_02630_b200.binding as B
+    from oracle import oracle as o
+
+    torch = G.torch_cuda()
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7720]))
+    key, icb = rng.bytes(16), rng.bytes(16)
+    data = np.frombuffer(rng.bytes(300000 + 9), dtype=np.uint8)
+    src, dst = G.to_device(data), G.device_empty(len(data))
+    other = torch.empty(1 << 20, dtype=torch.uint8, device="cuda:0")
+    other.fill_(1)               # first launch: lazy module loading happens here, not beside the engine
+    torch.cuda.synchronize()
+    ctx = B.aes_ctx_create(key)
+    B.aes_engine_start(0, idle_exit_ms=20000)
+    try:
+        t0 = time.time()
+        other.fill_(7)           # a kernel on torch's stream, beside 148 persistent CTAs
+        G.stream_sync()
+        assert time.time() - t0 < 5.0, "the fill had to wait for the engine"
+        B.aes_wait(B.aes_ctr_submit(ctx, icb, src.data_ptr(), dst.data_ptr(), len(data)))
+        assert dst.cpu().numpy().tobytes() == o.ctr(key, icb, data)
+        assert int(other[12345:12346].cpu().numpy()[0]) == 7
+    finally:
+        B.aes_engine_stop()
+    B.aes_ctx_destroy(ctx)
