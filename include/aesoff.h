@@ -226,6 +226,12 @@ typedef struct aes_loop_result {
 /* Returns AES_OK or the first error.  lat_ns: host, n*repeat doubles or NULL.      */
 int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res, double *lat_ns);
 
+/* The same from `nthreads` executor threads (1..64) at once: the n requests are split into
+ * contiguous shares, the window is divided among the threads, every thread runs the loop above
+ * on its share against the one shared ring.  With repeat > 1, lat_ns holds each thread's share
+ * back to back.  elapsed_ns is the wall time of all threads; max_in_flight the sum over threads. */
+int aes_loop_run_mt(const aes_loop_spec_t *spec, uint32_t nthreads, aes_loop_result_t *res, double *lat_ns);
+
 /* ---- calibration ---------------------------
  * Runs three microkernels with the engine's own table layout and launch shape and reports what the
  * units the cipher leans on deliver on this GPU: table lookups (PRMT + conflict-free LDS.32) per

@@ -95,6 +95,7 @@ def _load() -> ctypes.CDLL:
         "aes_host_free": (None, [vp]),
         "aes_loop_run": (i32, [vp, vp, vp]),
         "aes_openloop_run": (i32, [vp, vp, i32, vp, vp]),
+        "aes_loop_run_mt": (i32, [vp, ctypes.c_uint32, vp, vp]),
         "aes_calibrate": (i32, [i32, vp]),
     }
     for name, (res, args) in sigs.items():
@@ -107,7 +108,7 @@ def _load() -> ctypes.CDLL:
 _lib = _load()
 EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_ctx_create", "aes_ctx_destroy",
            "aes_ctx_round_keys", "aes_ctr_submit", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
-           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run", "aes_openloop_run", "aes_calibrate")
+           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run", "aes_loop_run_mt", "aes_openloop_run", "aes_calibrate")
 
 
 def aes_strerror(code: int) -> str:
@@ -217,7 +218,7 @@ def host_view(ptr: int, nbytes: int) -> np.ndarray:
 
 # ---- closed-loop executor ---------------------------------------------------------------------------
 def aes_loop_run(nonces, srcs, dsts, lens, window: int, ctx: int = 0, keys=None, keybits=None, repeat: int = 1,
-                 want_latency: bool = True) -> dict:
+                 want_latency: bool = True, threads: int = 1) -> dict:
     """Runs the native closed loop (see aes_loop_run in aesoff.h).  keys: n x 32 uint8 (16 used for
     128-bit keys) with keybits: n int32, or a shared ``ctx``.  Returns elapsed_ns, bytes, requests,
     ring_full_spins, max_in_flight and (optionally) lat_ns as a float64 array of n*repeat entries."""
@@ -238,8 +239,12 @@ def aes_loop_run(nonces, srcs, dsts, lens, window: int, ctx: int = 0, keys=None,
     spec.nonces, spec.srcs, spec.dsts, spec.lens = a_non.ctypes.data, a_src.ctypes.data, a_dst.ctypes.data, a_len.ctypes.data
     res = aes_loop_result_t()
     lat = np.zeros(n * repeat, dtype=np.float64) if want_latency else None
-    _check(_lib.aes_loop_run(ctypes.byref(spec), ctypes.byref(res), lat.ctypes.data if lat is not None else None),
-           "aes_loop_run")
+    if threads > 1:
+        _check(_lib.aes_loop_run_mt(ctypes.byref(spec), threads, ctypes.byref(res), lat.ctypes.data if lat is not None else None),
+               "aes_loop_run_mt")
+    else:
+        _check(_lib.aes_loop_run(ctypes.byref(spec), ctypes.byref(res), lat.ctypes.data if lat is not None else None),
+               "aes_loop_run")
     out = {k: getattr(res, k) for k, _ in aes_loop_result_t._fields_}
     out["lat_ns"] = lat
     return out

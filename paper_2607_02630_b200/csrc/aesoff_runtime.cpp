@@ -21,6 +21,7 @@
 #include <atomic>
 #include <deque>
 #include <mutex>
+#include <thread>
 #include <vector>
 
 #if defined(__x86_64__)
@@ -917,5 +918,51 @@ extern "C" int aes_openloop_run(const aes_loop_spec_t *spec, const uint64_t *arr
     res->elapsed_ns = now_ns() - t0;
     res->bytes = bytes;
     res->requests = done;
+    return AES_OK;
+}
+
+/* ============================================================================================ */
+/* closed loop from several executor threads ("worker pool")           */
+/* ============================================================================================ */
+extern "C" int aes_loop_run_mt(const aes_loop_spec_t *spec, uint32_t nthreads, aes_loop_result_t *res, double *lat_ns)
+{
+    if (!spec || !res || nthreads == 0 || nthreads > 64) return fail(AES_E_INVAL);
+    if (spec->n < nthreads) return fail(AES_E_INVAL);
+    std::vector<aes_loop_spec_t> specs(nthreads, *spec);
+    std::vector<aes_loop_result_t> results(nthreads);
+    std::vector<int> rcs(nthreads, AES_OK);
+    std::vector<std::thread> threads;
+    const size_t per = spec->n / nthreads;
+    const uint32_t window = spec->window / nthreads ? spec->window / nthreads : 1u;
+    const uint64_t t0 = now_ns();
+    for (uint32_t t = 0; t < nthreads; ++t) {
+        aes_loop_spec_t &s = specs[t];
+        const size_t first = per * t, count = (t + 1 == nthreads) ? spec->n - first : per;
+        s.n = count;
+        s.window = window;
+        s.nonces = spec->nonces + 16 * first;
+        s.srcs = spec->srcs + first;
+        s.dsts = spec->dsts + first;
+        s.lens = spec->lens + first;
+        if (spec->keys) {
+            s.keys = spec->keys + 32 * first;
+            s.keybits = spec->keybits + first;
+        }
+        double *lat = lat_ns ? lat_ns + first * (spec->repeat ? spec->repeat : 1) : nullptr;
+        threads.emplace_back([&, t, lat]() {
+            rcs[t] = aes_loop_run(&specs[t], &results[t], lat);
+            if (rcs[t] != AES_OK) rcs[t] = t_last_error ? t_last_error : rcs[t];
+        });
+    }
+    for (auto &th : threads) th.join();
+    memset(res, 0, sizeof(*res));
+    res->elapsed_ns = now_ns() - t0;
+    for (uint32_t t = 0; t < nthreads; ++t) {
+        if (rcs[t] != AES_OK) return fail(rcs[t]);
+        res->bytes += results[t].bytes;
+        res->requests += results[t].requests;
+        res->ring_full_spins += results[t].ring_full_spins;
+        res->max_in_flight += results[t].max_in_flight;
+    }
     return AES_OK;
 }
