@@ -415,27 +415,40 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
 
     if (lane == 0) P.hctl[AESOFF_CTL_ALIVE] = 1;
 
+    /* One poll = the next 8 (quiet) or 32 (busy) ring slots as 16-byte pieces, plus the stop word and two
+     * device counters.  piece g = 32 j + lane: slot g / 8 after the poll's first sequence number, piece g % 8.
+     * A poll is issued as soon as the previous one has been looked at, i.e. BEFORE that batch is processed:
+     * the PCIe round trip of the next batch runs under the on-chip work of this one.                       */
+    uint4 pc[8];
+    uint32_t p_stop = 0, p_nload = 2u;
+    unsigned long long p_idle = 0, p_reserved = 0;
+#define ISSUE_POLL(seq0)                                                                                     \
+    do {                                                                                                     \
+        p_nload = wide ? 8u : 2u;                                                                            \
+        _Pragma("unroll") for (uint32_t j = 0; j < 8; ++j)                                                  \
+        {                                                                                                    \
+            pc[j] = make_uint4(0, 0, 0, 0);                                                                  \
+            if (j < p_nload) {                                                                               \
+                const uint32_t k_ = j * 4u + (lane >> 3);                                                    \
+                const uint32_t sl_ = (uint32_t)(((seq0) + k_ - 1) & Rm);                                     \
+                pc[j] = ld_volatile_v4(reinterpret_cast<const uint8_t *>(P.hring + sl_) + 16u * (lane & 7u)); \
+            }                                                                                                \
+        }                                                                                                    \
+        if (lane == 0) {                                                                                     \
+            p_stop = ld_volatile_u32(P.hctl + AESOFF_CTL_STOP);                                              \
+            p_idle = *reinterpret_cast<volatile unsigned long long *>(g_idle);                               \
+            p_reserved = *reinterpret_cast<volatile unsigned long long *>(P.counters + AESOFF_CNT_TICKET);   \
+        }                                                                                                    \
+    } while (0)
+    bool repoll = true; /* the poll in flight (if any) does not start at next_seq */
+
     for (;;) {
         /* ---- phase 1: the PCIe round trip ---------------------------------------------------- */
-        /* piece g = 32 j + lane of the poll: slot g / 8 after next_seq, piece g % 8 of that slot */
-        uint4 pc[8];
-        const uint32_t nload = wide ? 8u : 2u;
-#pragma unroll
-        for (uint32_t j = 0; j < 8; ++j) {
-            pc[j] = make_uint4(0, 0, 0, 0);
-            if (j < nload) {
-                const uint32_t k = j * 4u + (lane >> 3);
-                const uint32_t sl = (uint32_t)((next_seq + k - 1) & Rm);
-                pc[j] = ld_volatile_v4(reinterpret_cast<const uint8_t *>(P.hring + sl) + 16u * (lane & 7u));
-            }
-        }
-        uint32_t stop = 0;
-        unsigned long long idle = 0, reserved = 0;
-        if (lane == 0) {
-            stop = ld_volatile_u32(P.hctl + AESOFF_CTL_STOP);
-            idle = *reinterpret_cast<volatile unsigned long long *>(g_idle);
-            reserved = *reinterpret_cast<volatile unsigned long long *>(P.counters + AESOFF_CNT_TICKET);
-        }
+        if (repoll) ISSUE_POLL(next_seq);
+        repoll = false;
+        const uint32_t nload = p_nload;
+        uint32_t stop = p_stop;
+        unsigned long long idle = p_idle, reserved = p_reserved;
 #pragma unroll
         for (uint32_t j = 0; j < 8; ++j) {
             if (j < nload) {
@@ -463,7 +476,10 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         idle = __shfl_sync(0xffffffffu, idle, 0);
         reserved = __shfl_sync(0xffffffffu, reserved, 0);
         wide = (n >= 8u) ? 1u : 0u;
+        const uint32_t n_seen = n;
+        if (n != 0) ISSUE_POLL(next_seq + n); /* the staged copy of this poll is in shared memory: pc[] is free */
         if (n == 0) {
+            repoll = true;
             if (stats_dirty) {
                 /* not on a request's way: a PCIe write in flight would hold up the next fence */
                 if (lane == 0) {
@@ -585,6 +601,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             base = nb;
         }
         if (lane >= n) nchunks = 0;
+        if (n != n_seen) repoll = true; /* the ticket ring took fewer requests than the poll in flight assumes */
         {   /* statistics for aes_engine_info */
             const uint32_t me = __ballot_sync(0xffffffffu, lane < n && (fine & AESOFF_FLAG_FINE));
             const uint32_t mh = __ballot_sync(0xffffffffu, lane < n && (fine & AESOFF_FLAG_HALF));
