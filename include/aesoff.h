@@ -125,8 +125,12 @@ int aes_engine_info(aes_engine_info_t *out);     /* host pointer; AES_OK / AES_E
  * asks for 128 and 256; 192 costs nothing more: Nk = 6, Nr = 12).
  * Returns NULL on error (AES_E_INVAL, AES_E_KEYBITS, AES_E_NOMEM).  Needs no GPU and
  * no running engine; cheap enough to sit on the request path (BASELINE.json
- * configs[3] creates one ctx per request).  The expanded key travels inside each
- * descriptor, so a ctx may be destroyed as soon as its last submit has returned. */
+ * configs[3] creates one ctx per request).  Where the expansion itself runs: on the
+ * DEVICE for the engine -- the first two submits of a ctx carry the raw key in their
+ * descriptor and the dispatcher warp expands it; the second also files the result in
+ * a device-side key table, which later submits only name -- and on the host, on
+ * demand, for aes_ctx_round_keys and the launch backend.  The key travels with the
+ * request, so a ctx may be destroyed as soon as its last submit has returned.      */
 aes_ctx_t *aes_ctx_create(const uint8_t *key, int keybits);
 void       aes_ctx_destroy(aes_ctx_t *ctx);      /* NULL is a no-op */
 

@@ -18,12 +18,13 @@
 
 struct aes_ctx {
     uint32_t rk[60]; /* round keys as little-endian-loaded words, zero padded (host expansion) */
-    int32_t nr;      /* 10 or 14 */
+    int32_t nr;      /* 10, 12 or 14 */
     int32_t keybits;
     uint32_t key[8]; /* the cipher key as little-endian-loaded words, zero padded */
     uint32_t state;  /* AESOFF_CTX_*, accessed atomically */
     uint32_t id;     /* ktab index once state >= INSTALLING */
     uint64_t epoch;  /* ktab generation the id belongs to */
+    uint32_t rk_ready; /* rk[] has been filled (lazily: the engine path expands keys on the device) */
 };
 
 const uint32_t *aesoff_T0_table();
