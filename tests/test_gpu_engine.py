@@ -404,3 +404,25 @@ def test_open_loop_executor_parity(P):
         for i in range(n):
             assert G.first_mismatch(dsts[i].cpu().numpy()[: len(datas[i])], wants[i]) == -1, "request %d" % i
     P.aes_ctx_destroy(ctx)
+
+
+def test_closed_loop_from_four_threads(P):
+    """aes_loop_run_mt: four executor threads share the ring ("worker pool"); every byte checked."""
+    import gpu_util as G
+
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 8000]))
+    n = 600
+    key = rng.bytes(32)
+    datas = [np.frombuffer(rng.bytes(int(rng.integers(1, 30000))), dtype=np.uint8) for _ in range(n)]
+    icbs = rng.integers(0, 256, size=(n, 16), dtype=np.uint8)
+    srcs = [G.to_device(d) for d in datas]
+    dsts = [G.device_empty(len(d)) for d in datas]
+    G.stream_sync()
+    ctx = P.aes_ctx_create(key)
+    r = P.aes_loop_run(icbs, [s.data_ptr() for s in srcs], [d.data_ptr() for d in dsts], [len(d) for d in datas],
+                       window=64, ctx=ctx, threads=4)
+    assert r["requests"] == n and r["bytes"] == sum(len(d) for d in datas) and (r["lat_ns"] > 0).all()
+    wants = G.oracle_many([(key, icbs[i].tobytes(), datas[i]) for i in range(n)])
+    for i in range(n):
+        assert G.first_mismatch(dsts[i].cpu().numpy()[: len(datas[i])], wants[i]) == -1, "request %d" % i
+    P.aes_ctx_destroy(ctx)
