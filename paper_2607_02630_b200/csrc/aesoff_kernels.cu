@@ -640,24 +640,24 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         }
         __threadfence(); /* descriptors and keys before the tickets that point at them */
         __syncwarp();
-        /* a request of up to four chunks (the fine-grained regime: every request of the poll) gets its
+        /* a request of up to eight chunks (the fine-grained regime: every request of the poll) gets its
          * tickets from its own lane; the warp then shares out the long ones, 32 tickets per step */
         if (lane < n) {
             const uint32_t rs = slot, md = fine << AESOFF_TICKET_MODE_SHIFT;
-            for (uint32_t ch = 0; ch < nchunks && ch < 4u; ++ch) {
+            for (uint32_t ch = 0; ch < nchunks && ch < 8u; ++ch) {
                 const unsigned long long tno = first_ticket + ch;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
                     make_uint4(rs, ch | md, keyloc, (uint32_t)tno + 1u);
             }
         }
-        for (uint32_t big = __ballot_sync(0xffffffffu, lane < n && nchunks > 4u); big; big &= big - 1u) {
+        for (uint32_t big = __ballot_sync(0xffffffffu, lane < n && nchunks > 8u); big; big &= big - 1u) {
             const uint32_t k = __ffs(big) - 1;
             const uint32_t nc = __shfl_sync(0xffffffffu, nchunks, k);
             const unsigned long long ft = __shfl_sync(0xffffffffu, first_ticket, k);
             const uint32_t kl = __shfl_sync(0xffffffffu, keyloc, k);
             const uint32_t md = __shfl_sync(0xffffffffu, fine, k) << AESOFF_TICKET_MODE_SHIFT;
             const uint32_t rs = (uint32_t)((next_seq + k - 1) & Rm);
-            for (uint32_t ch = 4u + lane; ch < nc; ch += 32) {
+            for (uint32_t ch = 8u + lane; ch < nc; ch += 32) {
                 const unsigned long long tno = ft + ch;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
                     make_uint4(rs, ch | md, kl, (uint32_t)tno + 1u);
