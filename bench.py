@@ -46,8 +46,10 @@ METRIC = "aes_ctr_payload_throughput"
 UNIT = "GB/s"
 
 # shared-memory lookups per 16-byte block in the CUDA path: per block
-# 1 (round 1) + 4 (round 2) + 16 * (Nr - 2) ; plus 27 per 8 blocks for the per-row constants
-LOOKUPS = {128: 1 + 4 + 16 * 8 + 27 / 8.0, 192: 1 + 4 + 16 * 10 + 27 / 8.0, 256: 1 + 4 + 16 * 12 + 27 / 8.0}
+# 1 (round 1) + 4 (round 2) + 16 * (Nr - 2); plus, per pair of consecutive rows (16 blocks per lane),
+# 27 for the first row's constants and 10 for stepping them to the second row
+SETUP = (27 + 10) / 16.0
+LOOKUPS = {128: 1 + 4 + 16 * 8 + SETUP, 192: 1 + 4 + 16 * 10 + SETUP, 256: 1 + 4 + 16 * 12 + SETUP}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the launch backend, from the ncu --set full captures
 # summarised in profiles/r1c_ncu.md (a persistent launch cannot be replayed by ncu)
 NCU_TRAFFIC = {

@@ -150,6 +150,7 @@ struct RowConst {
     uint32_t K1_0;                   /* round-1 column 0 without the T3[byte 15] term          */
     uint32_t K2_0, K2_1, K2_2, K2_3; /* round-2 columns without the terms fed by column 0      */
     uint32_t a3;                     /* address of T3[state byte 15] for last counter byte = lane */
+    uint32_t C1, s3;                 /* round-1 column 1 and round-0 word 3: all that counter byte 14 reaches */
 };
 
 /* U0..U3: the counter block with its last byte zero, as four little-endian-loaded words;
@@ -173,7 +174,25 @@ __device__ __forceinline__ RowConst row_setup(uint32_t ybase, const uint4 *rk4, 
     rc.K2_3 = TL(0, 0, C3) ^ TL(2, 2, C1) ^ TL(3, 3, C2) ^ k2.w;
     /* the last counter byte (lane + 32k) is xored into the table index: lane here, k per block */
     rc.a3 = taddr<3>(s3, ybase) ^ (lane << 8);
+    rc.C1 = C1;
+    rc.s3 = s3;
     return rc;
+}
+
+/* The next row of the same request when only counter byte 14 changed (no carry out of it): that byte
+ * enters round 1 through ONE lookup of column 1, and column 1 enters round 2 through one lookup per
+ * column -- 10 lookups (old and new term each) instead of the 27 of a full set-up.
+ * U3_new: word 3 of the new row's counter block (last byte zero), little-endian loaded.            */
+__device__ __forceinline__ void row_step(RowConst &rc, uint32_t ybase, uint32_t k0w, uint32_t U3_new)
+{
+    const uint32_t s3n = U3_new ^ k0w;
+    const uint32_t C1n = rc.C1 ^ TL(2, 2, rc.s3) ^ TL(2, 2, s3n);
+    rc.K2_0 ^= TL(1, 1, rc.C1) ^ TL(1, 1, C1n);
+    rc.K2_1 ^= TL(0, 0, rc.C1) ^ TL(0, 0, C1n);
+    rc.K2_2 ^= TL(3, 3, rc.C1) ^ TL(3, 3, C1n);
+    rc.K2_3 ^= TL(2, 2, rc.C1) ^ TL(2, 2, C1n);
+    rc.C1 = C1n;
+    rc.s3 = s3n; /* byte 3 of s3 (counter byte 15, zero here) is unchanged, and so is rc.a3 */
 }
 
 /* NB blocks per lane: L = lane + 32 (kb + b), b = 0..NB-1.
@@ -293,6 +312,39 @@ __device__ __forceinline__ void ctr_request_row(uint32_t ybase, const uint4 *rk4
     const uint32_t row_bytes = avail >= (int64_t)AESOFF_ROW_BYTES ? AESOFF_ROW_BYTES : (uint32_t)avail;
     const uint32_t lo_L = (m == 0) ? g.c0 : 0u;
     ctr_row<NB>(ybase, rk4, nr, U0, U1, U2, U3, src + row_off, dst + row_off, lo_L, row_bytes, lane, kb0, kb1);
+}
+
+/* `count` consecutive whole-row units of a request, rows m0, m0 + 1, ...: the first gets the full
+ * set-up, the following ones the 10-lookup step unless the increment carries out of counter byte 14. */
+template <int NB>
+__device__ __forceinline__ void ctr_request_rows(uint32_t ybase, const uint4 *rk4, int nr, const CtrGeom &g,
+                                                 const uint8_t *src, uint8_t *dst, uint64_t len, uint64_t m0,
+                                                 uint32_t count, uint32_t lane)
+{
+    RowConst rc;
+#pragma unroll 1
+    for (uint32_t r = 0; r < count; ++r) {
+        const uint64_t m = m0 + r;
+        const uint64_t l2 = g.lo_cleared + (m << 8);
+        const uint32_t U3 = bswap32((uint32_t)l2);
+        if (r == 0 || ((uint32_t)(l2 >> 8) & 0xffu) == 0u) {
+            const uint64_t h2 = g.hi + (l2 < g.lo_cleared ? 1ull : 0ull);
+            rc = row_setup(ybase, rk4, bswap32((uint32_t)(h2 >> 32)), bswap32((uint32_t)h2), bswap32((uint32_t)(l2 >> 32)),
+                           U3, lane);
+        } else {
+            row_step(rc, ybase, rk4[0].w, U3);
+        }
+        const int64_t row_off = ((int64_t)(m << 8) - (int64_t)g.c0) * 16;
+        const int64_t avail = (int64_t)len - row_off;
+        const uint32_t row_bytes = avail >= (int64_t)AESOFF_ROW_BYTES ? AESOFF_ROW_BYTES : (uint32_t)avail;
+        const uint32_t lo_L = (m == 0) ? g.c0 : 0u;
+#pragma unroll 1
+        for (uint32_t kb = 0; kb < 8; kb += NB) {
+            if (kb * 512u >= row_bytes) break;
+            if ((kb + NB) * 32u <= lo_L) continue;
+            row_blocks<NB>(rc, ybase, rk4, nr, src + row_off, dst + row_off, lo_L, row_bytes, lane, kb);
+        }
+    }
 }
 
 } /* namespace aesoff */

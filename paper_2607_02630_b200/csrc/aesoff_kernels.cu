@@ -203,14 +203,11 @@ __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase,
             const uint64_t m = (uint64_t)sl->unit0_row + (u >> 1);
             ctr_request_row<4>(ybase, rk4, nr, g, src, dst, len, m, lane, (u & 1u) * 4u, (u & 1u) * 4u + 4u);
         } else {
-            /* a whole-row unit is AESOFF_ROWS_PER_UNIT consecutive rows: half the claims and done counts */
-            const uint32_t crows_here = sl->n_rows;
-#pragma unroll 1
-            for (uint32_t rr = 0; rr < AESOFF_ROWS_PER_UNIT; ++rr) {
-                const uint32_t ri = u * AESOFF_ROWS_PER_UNIT + rr;
-                if (ri >= crows_here) break;
-                ctr_request_row<AESOFF_NB>(ybase, rk4, nr, g, src, dst, len, (uint64_t)sl->unit0_row + ri, lane);
-            }
+            /* a whole-row unit is AESOFF_ROWS_PER_UNIT consecutive rows: half the claims and done counts,
+             * and the second row's set-up is a 10-lookup step from the first's */
+            const uint32_t first = u * AESOFF_ROWS_PER_UNIT, crows_here = sl->n_rows;
+            const uint32_t cnt = crows_here - first < AESOFF_ROWS_PER_UNIT ? crows_here - first : AESOFF_ROWS_PER_UNIT;
+            ctr_request_rows<AESOFF_NB>(ybase, rk4, nr, g, src, dst, len, (uint64_t)sl->unit0_row + first, cnt, lane);
         }
         __syncwarp();
         if (lane == 0) {

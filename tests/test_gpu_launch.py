@@ -173,3 +173,37 @@ def test_calibration_microkernels(P):
     assert 26.0 <= c["round_lookups_per_clk_per_sm"] <= 32.5, c
     assert 1.7 <= c["alu_instr_per_clk_per_sm"] <= 2.1, c
     assert c["copy_gbs"] > 3000.0, c
+
+
+@pytest.mark.parametrize("low4", ["01fffe00", "01ffff00", "ffffff37", "ffffffff", "00000000", "a1b2ff9c"])
+def test_consecutive_rows_and_carries_out_of_counter_byte_14(P, low4):
+    """Whole-row units are two consecutive rows; the second row's set-up is derived from the first's unless the
+    increment carries out of counter byte 14.  96 MiB in one launch (the first 12,000 rows run as whole-row units),
+    ICBs whose bytes 12..15 put that carry on the first, the second, or no row of a unit, and a ragged first row:
+    the first 2 MiB in full and sampled windows against the oracle."""
+    import gpu_util as G
+
+    torch = G.torch_cuda()
+    n = (96 << 20) + 11
+    g = torch.Generator(device="cuda:0").manual_seed(workloads.SEED_BASE + 77)
+    src = torch.randint(0, 256, (n,), dtype=torch.uint8, device="cuda:0", generator=g)
+    dst = torch.empty_like(src)
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 6100]))
+    key = rng.bytes(16)
+    icb = rng.bytes(12) + bytes.fromhex(low4)
+    if low4 == "ffffffff":
+        icb = b"\xff" * 16  # the whole 128-bit counter wraps on the first increment
+    ctx = P.aes_ctx_create(key)
+    torch.cuda.synchronize()
+    P.aes_ctr_launch_batch([ctx], icb, [src.data_ptr()], [dst.data_ptr()], [n])
+    torch.cuda.synchronize()
+    P.aes_ctx_destroy(ctx)
+    W = 64 << 10
+    starts = list(range(0, 2 << 20, W)) + [n - W - 11] + [int(x) * 16 for x in rng.integers(0, (40 << 20) // 16, size=12)]
+    jobs, gots = [], []
+    for s0 in starts:
+        e0 = min(n, s0 + W + (11 if s0 == n - W - 11 else 0))
+        jobs.append((key, icb, src[s0:e0].cpu().numpy(), s0 // 16))
+        gots.append(dst[s0:e0].cpu().numpy())
+    for s0, got, want in zip(starts, gots, G.oracle_many(jobs)):
+        assert G.first_mismatch(got, want) == -1, "window at %d" % s0
