@@ -661,10 +661,11 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             }
         }
         const uint32_t total = __shfl_sync(0xffffffffu, incl, n - 1);
-        __threadfence();
         __syncwarp();
         published += total;
-        if (lane == 0 && total) st_release_gpu(g_published, published);
+        /* No fence here: the published count only tells the service warps how many tickets they may
+         * reserve; a ticket is taken when its own 16-byte word shows up (tag), whichever arrives first. */
+        if (lane == 0 && total) *reinterpret_cast<volatile unsigned long long *>(g_published) = published;
         /* an empty request (len == 0) has no ticket: complete it here */
         if (lane < n && nchunks == 0) {
             __threadfence_system();
