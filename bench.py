@@ -604,6 +604,13 @@ def extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, s
         lat["inflight_%d" % depth] = {"p50_us": percentile(a, 50), "p99_us": percentile(a, 99),
                                       "mean_us": float(a.mean()), "req_per_s": nl / (r["elapsed_ns"] * 1e-9)}
     res["latency_4KiB"] = lat
+    # ---- configs[0]: one 64 KiB AES-128 request, one in flight ----
+    w1 = workloads.config1()
+    n1 = 2000
+    r = B.aes_loop_run(np.repeat(w1.icb, n1, axis=0), [lsrc.data_ptr()] * n1, [ldst.data_ptr()] * n1, [65536] * n1, window=1, ctx=ctx)
+    a = r["lat_ns"][n1 // 20:] / 1e3
+    res["c1_64KiB_single"] = {"workload": w1.name, "p50_us": percentile(a, 50), "p99_us": percentile(a, 99),
+                              "payload_gbs": 65536.0 / (percentile(a, 50) * 1e3)}
     # same, payload in pinned HOST memory (the paper's j.buf): read and written over PCIe by the kernel
     hl = B.aes_host_alloc(2 * pool * small)
     hls = [hl + (i % pool) * small for i in range(nl)]
