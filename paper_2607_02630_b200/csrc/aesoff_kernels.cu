@@ -312,11 +312,15 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
         const bool ready = polled && tv.w == (uint32_t)t + 1u;
         const uint32_t ready_mask = __ballot_sync(0xffffffffu, ready);
         if (ready_mask) {
-            __threadfence(); /* acquire: the dispatcher's dq/ktab writes precede its ticket stores */
-            const uint32_t ring = tv.x, chunk = tv.y & AESOFF_TICKET_CHUNK_MASK, keyloc = tv.z;
+            /* The expanded key is ordered before the ticket by the dispatcher's fence (only requests that
+             * brought a raw key pay for one); the descriptor is not: its 8 pieces carry the request's
+             * sequence number and a piece read too early is simply read again.                          */
+            __threadfence();
+            const uint32_t seq32 = tv.x, chunk = tv.y & AESOFF_TICKET_CHUNK_MASK, keyloc = tv.z;
+            const uint32_t ring = (seq32 - 1u) & (P.R - 1u);
             const uint32_t unit_mode = tv.y >> AESOFF_TICKET_MODE_SHIFT; /* AESOFF_FLAG_FINE / _HALF / 0 */
-            /* descriptor (lanes 0..5) and expanded key (lanes 8..22), 16 B each; four slots' loads are in
-             * flight together (one L2 round trip per four slots, not per slot)                          */
+            /* descriptor pieces (lanes 0..7) and expanded key (lanes 8..22), 16 B each; four slots' loads are
+             * in flight together (one L2 round trip per four slots, not per slot)                        */
             for (uint32_t m = ready_mask; m;) {
                 uint32_t sj[4];
                 uint4 v[4];
@@ -328,24 +332,39 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
                         m &= m - 1u;
                     }
                 }
+                for (;;) {
+                    bool stale = false;
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
-                    if (sj[q] < 32u) {
-                        const uint32_t rj = __shfl_sync(0xffffffffu, ring, sj[q]);
-                        const uint32_t kj = __shfl_sync(0xffffffffu, keyloc, sj[q]);
-                        if (lane < AESOFF_DESC_BYTES / 16)
-                            v[q] = __ldcg(reinterpret_cast<const uint4 *>(P.dq + rj) + lane);
-                        else if (lane >= 8 && lane < 8 + 15)
-                            v[q] = __ldcg(reinterpret_cast<const uint4 *>(P.ktab + kj) + (lane - 8));
+                    for (int q = 0; q < 4; ++q) {
+                        if (sj[q] < 32u) {
+                            const uint32_t rj = __shfl_sync(0xffffffffu, ring, sj[q]);
+                            const uint32_t kj = __shfl_sync(0xffffffffu, keyloc, sj[q]);
+                            if (lane < 8)
+                                v[q] = ld_volatile_v4(reinterpret_cast<const uint4 *>(P.dq + rj) + lane);
+                            else if (lane < 8 + 15)
+                                v[q] = __ldcg(reinterpret_cast<const uint4 *>(P.ktab + kj) + (lane - 8));
+                        }
                     }
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        if (sj[q] < 32u) {
+                            const uint32_t want = __shfl_sync(0xffffffffu, seq32, sj[q]);
+                            if (lane < 8 && v[q].w != want) stale = true;
+                        }
+                    }
+                    if (!__any_sync(0xffffffffu, stale)) break;
                 }
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     if (sj[q] < 32u) {
-                        if (lane < AESOFF_DESC_BYTES / 16)
-                            reinterpret_cast<uint4 *>(&c->slot[sj[q]].desc)[lane] = v[q];
-                        else if (lane >= 8 && lane < 8 + 15)
+                        if (lane < 8) {
+                            uint32_t *dw = reinterpret_cast<uint32_t *>(&c->slot[sj[q]].desc) + 3u * lane;
+                            dw[0] = v[q].x;
+                            dw[1] = v[q].y;
+                            dw[2] = v[q].z;
+                        } else if (lane < 8 + 15) {
                             c->slot[sj[q]].rk4[lane - 8] = v[q];
+                        }
                     }
                 }
             }
@@ -504,8 +523,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         last_activity = globaltimer_ns();
 
         /* ---- phase 2: lane k derives the geometry of request next_seq + k ---------------------- */
-        uint32_t icb[4] = {0, 0, 0, 0};
-        unsigned long long src = 0, dst = 0, len = 0, rows = 0;
+        unsigned long long len = 0, rows = 0;
         uint32_t nchunks = 0, crows = P.chunk_rows, fine = 0, nr = 0;
         /* Latency modes.  A request of up to 64 KiB is always cut into 1/8-row units (32 blocks per
          * warp; it is submission-bound anyway).  A larger one, up to fine_rows rows, is cut by the
@@ -521,16 +539,11 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         const unsigned long long warps = (unsigned long long)gridDim.x * AESOFF_WORKER_WARPS;
         if (lane < n) {
 #define PW(p) sw[AESOFF_PW_INDEX(p)]
-            icb[0] = PW(AESOFF_PW_ICB + 0);
-            icb[1] = PW(AESOFF_PW_ICB + 1);
-            icb[2] = PW(AESOFF_PW_ICB + 2);
-            icb[3] = PW(AESOFF_PW_ICB + 3);
-            src = ((unsigned long long)PW(AESOFF_PW_SRC + 1) << 32) | PW(AESOFF_PW_SRC);
-            dst = ((unsigned long long)PW(AESOFF_PW_DST + 1) << 32) | PW(AESOFF_PW_DST);
+            /* only what the geometry needs; the rest goes from the staging area straight into dq */
             len = ((unsigned long long)PW(AESOFF_PW_LEN + 1) << 32) | PW(AESOFF_PW_LEN);
             nr = kw >> 24;
             const unsigned long long nblocks = (len >> 4) + ((len & 15ull) ? 1ull : 0ull);
-            const uint32_t c0 = icb[3] >> 24;
+            const uint32_t c0 = PW(AESOFF_PW_ICB + 3) >> 24;
             rows = nblocks ? ((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0ull;
         }
         /* rows of this poll up to and including request k */
@@ -586,7 +599,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             }
             unsigned long long nb = published;
             if (lane == 0 && oldest < next_seq)
-                nb = *reinterpret_cast<volatile uint64_t *>(&P.dq[(oldest - 1) & Rm].first_ticket);
+                nb = *reinterpret_cast<volatile uint64_t *>(&P.dq[(oldest - 1) & Rm].w[24]); /* first_ticket: words 18, 19 */
             nb = __shfl_sync(0xffffffffu, nb, 0);
             if (nb == base) {
                 if (nfit > 0) {
@@ -623,28 +636,32 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             else
                 key_expand<8>(ybase, key, P.ktab[keyloc].rk);
         }
-#undef PW
         if (lane < n) {
-            aesoff_dev_desc_t *d = P.dq + slot;
-            uint4 *d4 = reinterpret_cast<uint4 *>(d);
-            d4[0] = make_uint4(icb[0], icb[1], icb[2], icb[3]);
-            d4[1] = make_uint4((uint32_t)src, (uint32_t)(src >> 32), (uint32_t)dst, (uint32_t)(dst >> 32));
-            d4[2] = make_uint4((uint32_t)len, (uint32_t)(len >> 32), nr, fine);
-            d4[3] = make_uint4(nchunks, crows, (uint32_t)s, (uint32_t)(s >> 32));
-            d4[4] = make_uint4((uint32_t)rows, (uint32_t)(rows >> 32), (uint32_t)first_ticket,
-                               (uint32_t)(first_ticket >> 32));
-            d4[5] = make_uint4(keyloc, 0u, 0u, 0u);
+            /* the 24 descriptor words as 8 pieces of {3 words, tag}: see aesoff_dq_entry_t */
+            uint4 *d4 = reinterpret_cast<uint4 *>(P.dq + slot);
+            const uint32_t tg = (uint32_t)s;
+            d4[0] = make_uint4(PW(AESOFF_PW_ICB + 0), PW(AESOFF_PW_ICB + 1), PW(AESOFF_PW_ICB + 2), tg);
+            d4[1] = make_uint4(PW(AESOFF_PW_ICB + 3), PW(AESOFF_PW_SRC), PW(AESOFF_PW_SRC + 1), tg);
+            d4[2] = make_uint4(PW(AESOFF_PW_DST), PW(AESOFF_PW_DST + 1), (uint32_t)len, tg);
+            d4[3] = make_uint4((uint32_t)(len >> 32), nr, fine, tg);
+            d4[4] = make_uint4(nchunks, crows, (uint32_t)s, tg);
+            d4[5] = make_uint4((uint32_t)(s >> 32), (uint32_t)rows, (uint32_t)(rows >> 32), tg);
+            d4[6] = make_uint4((uint32_t)first_ticket, (uint32_t)(first_ticket >> 32), keyloc, tg);
+            d4[7] = make_uint4(0u, 0u, 0u, tg);
         }
-        __threadfence(); /* descriptors and keys before the tickets that point at them */
+#undef PW
+        /* expanded keys (if any request of this poll brought a raw one) before the tickets that point at
+         * them; descriptors need no fence, their pieces validate themselves */
+        if (__any_sync(0xffffffffu, lane < n && (kw & AESOFF_KW_RAW))) __threadfence();
         __syncwarp();
         /* a request of up to eight chunks (the fine-grained regime: every request of the poll) gets its
          * tickets from its own lane; the warp then shares out the long ones, 32 tickets per step */
         if (lane < n) {
-            const uint32_t rs = slot, md = fine << AESOFF_TICKET_MODE_SHIFT;
+            const uint32_t md = fine << AESOFF_TICKET_MODE_SHIFT;
             for (uint32_t ch = 0; ch < nchunks && ch < 8u; ++ch) {
                 const unsigned long long tno = first_ticket + ch;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
-                    make_uint4(rs, ch | md, keyloc, (uint32_t)tno + 1u);
+                    make_uint4((uint32_t)s, ch | md, keyloc, (uint32_t)tno + 1u);
             }
         }
         for (uint32_t big = __ballot_sync(0xffffffffu, lane < n && nchunks > 8u); big; big &= big - 1u) {
@@ -653,11 +670,11 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             const unsigned long long ft = __shfl_sync(0xffffffffu, first_ticket, k);
             const uint32_t kl = __shfl_sync(0xffffffffu, keyloc, k);
             const uint32_t md = __shfl_sync(0xffffffffu, fine, k) << AESOFF_TICKET_MODE_SHIFT;
-            const uint32_t rs = (uint32_t)((next_seq + k - 1) & Rm);
+            const uint32_t sq = (uint32_t)(next_seq + k);
             for (uint32_t ch = 8u + lane; ch < nc; ch += 32) {
                 const unsigned long long tno = ft + ch;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
-                    make_uint4(rs, ch | md, kl, (uint32_t)tno + 1u);
+                    make_uint4(sq, ch | md, kl, (uint32_t)tno + 1u);
             }
         }
         const uint32_t total = __shfl_sync(0xffffffffu, incl, n - 1);

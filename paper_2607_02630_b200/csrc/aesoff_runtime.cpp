@@ -70,7 +70,7 @@ struct Engine {
     aesoff_host_slot_t *hring = nullptr; /* pinned, mapped */
     uint64_t *hmail = nullptr;           /* pinned, mapped */
     uint32_t *hctl = nullptr;            /* pinned, mapped */
-    aesoff_dev_desc_t *dq = nullptr;
+    aesoff_dq_entry_t *dq = nullptr;
     aesoff_key_t *ktab = nullptr;
     aesoff_ticket_t *tmap = nullptr;
     uint64_t *counters = nullptr, *dev_done_seq = nullptr;
@@ -322,7 +322,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     ok = ok && cudaHostAlloc((void **)&e.hring, (size_t)e.R * sizeof(aesoff_host_slot_t), hflags) == cudaSuccess;
     ok = ok && cudaHostAlloc((void **)&e.hmail, (size_t)e.R * 8, hflags) == cudaSuccess;
     ok = ok && cudaHostAlloc((void **)&e.hctl, AESOFF_CTL_WORDS * 4, hflags) == cudaSuccess;
-    ok = ok && cudaMalloc((void **)&e.dq, (size_t)e.R * sizeof(aesoff_dev_desc_t)) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.dq, (size_t)e.R * sizeof(aesoff_dq_entry_t)) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.tmap, (size_t)e.TM * sizeof(aesoff_ticket_t)) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.ktab, (size_t)(AESOFF_KEY_IDS + e.R) * sizeof(aesoff_key_t)) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.counters, AESOFF_CNT_WORDS * 8) == cudaSuccess;
@@ -336,6 +336,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     memset(e.hring, 0, (size_t)e.R * sizeof(aesoff_host_slot_t));
     memset(e.hmail, 0, (size_t)e.R * 8);
     ok = ok && cudaMemset(e.dev_done_seq, 0, (size_t)e.R * 8) == cudaSuccess;
+    ok = ok && cudaMemset(e.dq, 0, (size_t)e.R * sizeof(aesoff_dq_entry_t)) == cudaSuccess; /* no tag matches yet */
     ok = ok && cudaMemcpy(e.dT0, aesoff_T0_table(), 256 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
     if (ok) reset_key_ids(e);
     }
@@ -658,7 +659,7 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         L.blob = nullptr;
         L.cap_req = R > L.cap_req ? R : L.cap_req;
         L.cap_tickets = TM > L.cap_tickets ? TM : L.cap_tickets;
-        L.blob_bytes = AESOFF_CNT_WORDS * 8 + L.cap_req * (sizeof(aesoff_dev_desc_t) + sizeof(aesoff_key_t)) +
+        L.blob_bytes = AESOFF_CNT_WORDS * 8 + L.cap_req * (sizeof(aesoff_dq_entry_t) + sizeof(aesoff_key_t)) +
                        L.cap_tickets * sizeof(aesoff_ticket_t);
         bool ok = true;
         ok = ok && cudaMalloc((void **)&L.blob, L.blob_bytes) == cudaSuccess;
@@ -684,9 +685,10 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     }
     /* blob layout for this call (every part a multiple of 16 bytes) */
     const size_t off_dq = AESOFF_CNT_WORDS * 8;
-    const size_t off_key = off_dq + n * sizeof(aesoff_dev_desc_t);
+    const size_t off_key = off_dq + n * sizeof(aesoff_dq_entry_t);
     uint64_t *hc = reinterpret_cast<uint64_t *>(L.stage);
-    aesoff_dev_desc_t *hd = reinterpret_cast<aesoff_dev_desc_t *>(L.stage + off_dq);
+    std::vector<aesoff_dev_desc_t> hd(n); /* packed into tagged dq entries below */
+    aesoff_dq_entry_t *hq = reinterpret_cast<aesoff_dq_entry_t *>(L.stage + off_dq);
     aesoff_key_t *hk = reinterpret_cast<aesoff_key_t *>(L.stage + off_key);
     size_t nkeys = 0;
     for (size_t i = 0; i < n; ++i) {
@@ -725,13 +727,22 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
             aesoff_ticket_t &tk = ht[t + c];
             const uint64_t left = all_rows - (rows_before + (uint64_t)c * crows[i]); /* rows from this chunk on */
             const uint32_t mode = left <= wave ? AESOFF_FLAG_FINE : left <= 5 * wave ? AESOFF_FLAG_HALF : 0u;
-            tk.ring = (uint32_t)i;
+            tk.seq32 = (uint32_t)(i + 1);
             tk.chunk = c | (mode << AESOFF_TICKET_MODE_SHIFT);
             tk.keyloc = hd[i].keyloc;
             tk.tag = (uint32_t)(t + c) + 1u;
         }
         t += nch[i];
         rows_before += rows[i];
+    }
+    for (size_t i = 0; i < n; ++i) { /* the 24 descriptor words as 8 pieces of {3 words, tag = seq} */
+        const uint32_t *w = reinterpret_cast<const uint32_t *>(&hd[i]);
+        for (int q = 0; q < 8; ++q) {
+            hq[i].w[4 * q + 0] = w[3 * q + 0];
+            hq[i].w[4 * q + 1] = w[3 * q + 1];
+            hq[i].w[4 * q + 2] = w[3 * q + 2];
+            hq[i].w[4 * q + 3] = (uint32_t)(i + 1);
+        }
     }
     memset(hc, 0, AESOFF_CNT_WORDS * 8);
     hc[AESOFF_CNT_PUBLISHED] = total;
@@ -752,7 +763,7 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     aesoff_params_t p;
     memset(&p, 0, sizeof(p));
     p.counters = reinterpret_cast<uint64_t *>(L.blob);
-    p.dq = reinterpret_cast<aesoff_dev_desc_t *>(L.blob + off_dq);
+    p.dq = reinterpret_cast<aesoff_dq_entry_t *>(L.blob + off_dq);
     p.ktab = reinterpret_cast<aesoff_key_t *>(L.blob + off_key);
     p.tmap = reinterpret_cast<aesoff_ticket_t *>(L.blob + off_tk);
     p.dq_done = L.dq_done;

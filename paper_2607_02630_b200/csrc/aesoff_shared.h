@@ -8,12 +8,12 @@
  *                host writes each piece with ONE 16-byte store, the dispatcher reads each with
  *                ONE 16-byte load, so a piece is either the old one or the new one and the whole
  *                descriptor arrives in a single PCIe round trip (no flag-then-body).   step a2
- *   dq           device memory, R descriptors of 96 B: the request plus the chunk geometry
- *                the dispatcher derived.                                               step a3
+ *   dq           device memory, R descriptors of 128 B (96 B of fields as 8 tagged pieces): the
+ *                request plus the chunk geometry the dispatcher derived.                step a3
  *   ktab         device memory, (AESOFF_KEY_IDS + R) expanded keys of 256 B: entries below
  *                AESOFF_KEY_IDS belong to contexts that have been installed, the rest to ring
  *                slots (keys of one-shot contexts, expanded on the device).            step a1
- *   tmap         device memory ring of 2^k 16-byte tickets {ring slot, chunk, key index, tag}.
+ *   tmap         device memory ring of 2^k 16-byte tickets {seq low half, chunk, key index, tag}.
  *   mailbox      pinned, host-mapped, R x 8 B: slot -> last completed seq.             step a7
  */
 #ifndef AESOFF_SHARED_H
@@ -98,6 +98,14 @@ typedef struct __attribute__((aligned(16))) aesoff_dev_desc {
     uint32_t pad[3];
 } aesoff_dev_desc_t;       /* 96 bytes */
 
+/* dq entry in device memory: the 24 words of aesoff_dev_desc_t as 8 pieces of {3 words, tag}, tag = low 32
+ * bits of the request's sequence number -- self-validating like a host ring slot, so that the dispatcher
+ * needs no fence between writing a descriptor and writing the tickets that point at it: a service warp that
+ * reads a piece too early sees a wrong tag and reads again.                                              */
+typedef struct __attribute__((aligned(128))) aesoff_dq_entry {
+    uint32_t w[32];        /* word p (0..23) of the descriptor at w[(p / 3) * 4 + p % 3], tags at w[4q + 3] */
+} aesoff_dq_entry_t;       /* 128 bytes */
+
 typedef struct __attribute__((aligned(16))) aesoff_key {
     uint32_t rk[60];       /* round keys, word c of round r at rk[4r+c], little-endian load of the
                               FIPS-197 byte string (byte 0 of the word = row 0 of column c)            */
@@ -107,7 +115,8 @@ typedef struct __attribute__((aligned(16))) aesoff_key {
 #define AESOFF_TICKET_CHUNK_MASK 0x0fffffffu
 #define AESOFF_TICKET_MODE_SHIFT 28u
 typedef struct __attribute__((aligned(16))) aesoff_ticket {
-    uint32_t ring;         /* index of the request in dq / mailbox                                     */
+    uint32_t seq32;        /* low 32 bits of the request's sequence number: (seq32 - 1) & (R - 1) is its
+                              index in dq / mailbox, and seq32 the tag its dq pieces must carry         */
     uint32_t chunk;        /* bits 0..27 chunk index; bits 28..29 unit size of this chunk:
                               0 rows, AESOFF_FLAG_FINE 1/8 rows, AESOFF_FLAG_HALF half rows            */
     uint32_t keyloc;
@@ -118,7 +127,7 @@ typedef struct aesoff_params {
     aesoff_host_slot_t *hring;      /* host-mapped (persistent mode)                     */
     volatile uint64_t  *hmail;      /* host-mapped mailbox, may be NULL in drain mode    */
     volatile uint32_t  *hctl;       /* host-mapped control words, NULL in drain mode     */
-    aesoff_dev_desc_t  *dq;
+    aesoff_dq_entry_t  *dq;
     aesoff_key_t       *ktab;
     aesoff_ticket_t    *tmap;
     uint64_t           *counters;
