@@ -119,7 +119,7 @@ __device__ __forceinline__ uint32_t sub_word(uint32_t w, uint32_t ybase)
  * and Rcon lands in the low byte.  One thread, one serial chain of 10 (Nk = 4), 8 (Nk = 6) or 13
  * (Nk = 8) SubWords: well under a microsecond, against a PCIe round trip for shipping 240 bytes. */
 template <int NK>
-__device__ __noinline__ void key_expand(uint32_t ybase, const uint32_t *key, uint32_t *out)
+__device__ __forceinline__ void key_expand(uint32_t ybase, const uint32_t *key, uint32_t *out)
 {
     uint32_t w[NK];
 #pragma unroll

@@ -42,7 +42,7 @@ def test_engine_kernel_has_no_spills_and_96_registers(cubin):
     stack, st, ld, regs = map(int, m.groups())
     assert st == 0 and ld == 0, "the engine kernel spills (%d B stores, %d B loads): see this file's docstring" % (st, ld)
     assert regs <= 96, regs
-    assert stack <= 64, stack  # the dispatcher's raw-key array only
+    assert stack <= 64, stack
 
 
 def test_sass_has_the_instructions_the_design_rests_on(cubin):
