@@ -214,6 +214,9 @@ def main():
     ap.add_argument("--backend", default="engine", choices=["engine", "launch"])
     ap.add_argument("--workload", default="c2", choices=["c2", "c3"])
     ap.add_argument("--chunk-rows", type=int, default=0)
+    ap.add_argument("--launch-requests", type=int, default=0,
+                    help="--backend launch: requests per ordinary launch (0 = the config's in-flight window; the whole "
+                         "batch in ONE launch is the operating point the ncu captures under profiles/ are made at)")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e / latency / cpu_baseline / kernel-only legs")
     ap.add_argument("--sweep", action="store_true", help="configs[4]: size x in-flight x key-size table (one GPU)")
     ap.add_argument("--sweep-out", default="", help="with --sweep / --openloop: also write the table to this JSON file")
@@ -283,7 +286,7 @@ def main():
         r = B.aes_loop_run(w.icb, srcs, dsts, lens, window=w.in_flight, ctx=ctx, want_latency=False)
         assert r["requests"] == n
 
-    LB = w.in_flight  # requests per ordinary launch in the launch backend
+    LB = args.launch_requests or w.in_flight  # requests per ordinary launch in the launch backend
 
     def step_launch(stream_ptr, events=None):
         for b0 in range(0, n, LB):

@@ -27,6 +27,13 @@
  *     the code in a thread-local slot read by aes_last_error().  Nothing aborts,
  *     nothing throws.  There is NO CPU fallback: without a CUDA device every
  *     compute call fails with AES_E_CUDA.
+ *   - Key hygiene and side channels.  aes_ctx_destroy wipes the context; ring slots,
+ *     the device key table and the launch backend's staging blob are wiped when they
+ *     are freed.  The cipher is table based (T-tables in shared memory, FIPS-197
+ *     sec. 5.1 folded): its memory access pattern depends on key and data, as in
+ *     every table-based AES.  Each lane reads only its own bank, so there are no
+ *     data-dependent bank conflicts inside a warp, but this is NOT a constant-time
+ *     implementation and must not share a GPU with an adversary that can time it.
  */
 #ifndef AESOFF_H
 #define AESOFF_H
@@ -90,12 +97,21 @@ typedef struct aes_engine_opts {
  * (it leaves 1,472 threads and 10 K registers per SM), with one catch: the FIRST
  * launch of a kernel whose module CUDA has not loaded yet (lazy loading) blocks
  * until the engine stops -- launch every kernel once before aes_engine_start, or
- * run with CUDA_MODULE_LOADING=EAGER.                                              */
+ * run with CUDA_MODULE_LOADING=EAGER.
+ * The persistent engine cannot run under a tool that serialises launches (ncu,
+ * compute-sanitizer, CUDA_LAUNCH_BLOCKING=1): the launch call then waits for a
+ * kernel that waits for submissions.  With idle_exit_ms set the kernel leaves by
+ * itself and this call returns AES_E_STOPPED (never AES_OK for an engine that has
+ * already exited); with idle_exit_ms == 0 it would not return.  Profile through
+ * aes_ctr_launch_batch (the same worker code as an ordinary launch).              */
 int aes_engine_start(int device, const aes_engine_opts_t *opts);
 
-/* Waits for every accepted request to complete, makes the persistent kernel exit,
- * frees ring and mailbox.  Handles issued before the stop keep answering
- * aes_poll() == 1.  Returns AES_OK or AES_E_STOPPED / AES_E_CUDA.                 */
+/* Refuses new submissions, lets the aes_ctr_submit calls already past that check
+ * finish publishing, waits for every accepted request to complete and makes the
+ * persistent kernel exit.  Ring and mailbox are kept for the next start.  Handles
+ * issued before a clean stop keep answering aes_poll() == 1; if the kernel had died
+ * (AES_E_STOPPED is returned) the requests it never completed answer AES_E_STOPPED.
+ * Returns AES_OK or AES_E_STOPPED / AES_E_CUDA.                                     */
 int aes_engine_stop(void);
 
 typedef struct aes_engine_info {
@@ -168,7 +184,10 @@ aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16],
  * Wait-free: one acquire load of the host-mapped mailbox.  Once it has returned 1,
  * every byte of dst is visible to any copy or kernel issued afterwards on any
  * stream of the device, and to the host if dst is host memory.
- * aes_wait: spins on aes_poll for at most timeout_ns (UINT64_MAX = forever).
+ * aes_wait: polls for at most timeout_ns (UINT64_MAX = forever): busy (pause) for the
+ * first ~20 us -- the offloads this engine is built for take 10 -- then yielding the
+ * core, then sleeping in steps that grow to 50 us, so that a pool of executor threads
+ * waiting on long requests does not burn a core each.
  * Returns AES_OK, AES_E_TIMEOUT or the aes_poll error.                             */
 int aes_poll(aes_handle_t h);
 int aes_wait(aes_handle_t h, uint64_t timeout_ns);

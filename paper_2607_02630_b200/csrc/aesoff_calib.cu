@@ -37,6 +37,8 @@ calib_lookup_kernel(const uint32_t *T0, uint32_t iters, uint32_t *sink, unsigned
     uint32_t x[CALIB_CHAINS];
 #pragma unroll
     for (int i = 0; i < CALIB_CHAINS; ++i) x[i] = (threadIdx.x * 2654435761u) ^ (i * 0x9e3779b9u) ^ blockIdx.x;
+    unsigned long long g0, g1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g0));
     const long long t0 = clock64();
     for (uint32_t it = 0; it < iters; ++it) {
         if (with_loads == 2) {
@@ -71,11 +73,15 @@ calib_lookup_kernel(const uint32_t *T0, uint32_t iters, uint32_t *sink, unsigned
         }
     }
     const long long t1 = clock64();
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(g1));
     uint32_t acc = 0;
 #pragma unroll
     for (int i = 0; i < CALIB_CHAINS; ++i) acc ^= x[i];
     if (acc == 0x12345678u) sink[0] = acc; /* keeps the chains alive */
-    if (threadIdx.x == 0) cycles[blockIdx.x] = (unsigned long long)(t1 - t0);
+    if (threadIdx.x == 0) {
+        cycles[blockIdx.x] = (unsigned long long)(t1 - t0);
+        cycles[gridDim.x + blockIdx.x] = g1 - g0; /* nanoseconds of the same interval: the SM clock is their ratio */
+    }
 }
 
 __global__ void __launch_bounds__(CALIB_THREADS, 2) calib_copy_kernel(const uint4 *src, uint4 *dst, size_t n16)
@@ -102,7 +108,7 @@ extern "C" int aesoff_run_calibration(int device, double out[6])
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
     bool ok = cudaMalloc(&dT0, 1024) == cudaSuccess && cudaMalloc(&sink, 16) == cudaSuccess &&
-              cudaMalloc(&cyc, sizeof(unsigned long long) * sms) == cudaSuccess;
+              cudaMalloc(&cyc, sizeof(unsigned long long) * 2 * sms) == cudaSuccess;
     ok = ok && cudaMemcpy(dT0, aesoff_T0_table(), 1024, cudaMemcpyHostToDevice) == cudaSuccess;
     const size_t smem = 196608;
     ok = ok && cudaFuncSetAttribute(calib_lookup_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) == cudaSuccess;
@@ -114,15 +120,17 @@ extern "C" int aesoff_run_calibration(int device, double out[6])
         calib_lookup_kernel<<<sms, CALIB_THREADS, smem>>>(dT0, iters, sink, cyc, with_loads);
         cudaEventRecord(e1);
         ok = cudaEventSynchronize(e1) == cudaSuccess;
-        unsigned long long c0 = 0;
+        unsigned long long c0 = 0, ns0 = 0;
         ok = ok && cudaMemcpy(&c0, cyc, sizeof(c0), cudaMemcpyDeviceToHost) == cudaSuccess;
+        ok = ok && cudaMemcpy(&ns0, cyc + sms, sizeof(ns0), cudaMemcpyDeviceToHost) == cudaSuccess;
         float ms = 0;
         cudaEventElapsedTime(&ms, e0, e1);
         /* per CTA: 16 warps x iters x 16 lookups (warp-wide) in c0 cycles */
         const double ops = (double)(CALIB_THREADS / 32) * iters * CALIB_CHAINS;
         /* alu: 4 PRMT + 4 LOP3 per 4 chains; round: 16 lookups per 4 chains */
         res[mode] = with_loads == 1 ? ops / (double)c0 : with_loads == 0 ? ops * 2.0 / (double)c0 : ops * 4.0 / (double)c0;
-        if (with_loads == 1) mhz = (double)c0 / (ms * 1e3);
+        /* in-kernel cycles over in-kernel globaltimer nanoseconds (an event time would include launch and table fill) */
+        if (with_loads == 1 && ns0) mhz = (double)c0 * 1e3 / (double)ns0;
     }
     /* copy: 2 x 1 GiB, three passes, best */
     double copy_gbs = 0;

@@ -1,10 +1,10 @@
 /*
  * aesoff_keys.cpp -- host-side key expansion and the T0 table of the product library.
  *
- * Step a1 of the path: FIPS-197 sec. 5.2 KeyExpansion(), run by aes_ctx_create().  It stays on
- * the host because its 40-52 S-box steps are one serial dependency chain (about 100 ns here,
- * microseconds on one GPU thread) and because the expanded key travels inside the descriptor, so
- * the GPU needs no per-context state.  This file shares nothing with oracle/: the S-box below is
+ * Step a1 of the path: FIPS-197 sec. 5.2 KeyExpansion().  On the engine path the expansion runs on the
+ * DEVICE (the raw key rides in the descriptor, key_expand<NK> in aesoff_cipher.cuh); the host copy below
+ * serves aes_ctx_round_keys() (so that tests can pin the schedule on its own) and the launch backend, which
+ * ships expanded keys in its one host->device blob.  This file shares nothing with oracle/: the S-box below is
  * built from discrete logarithms to the generator {03} (a different route from the oracle's
  * search for inverses), so a slip in either shows up as a parity failure.
  */

@@ -16,8 +16,10 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <sched.h>
 #include <time.h>
 
+#include <algorithm>
 #include <atomic>
 #include <deque>
 #include <mutex>
@@ -83,6 +85,16 @@ struct Engine {
     std::mutex id_mu;
     std::deque<std::pair<uint32_t, uint64_t>> id_free; /* (index, next_seq when freed), FIFO   */
     std::atomic<uint64_t> k_epoch{1};     /* bumped whenever ktab is (re)allocated             */
+    /* aes_ctr_submit calls between their `running` check and their last slot store: aes_engine_stop waits
+     * for this to reach 0 before it reads next_seq, so no sequence number is published behind its back */
+    std::atomic<int> submitters{0};
+    /* every sequence number below this belongs to a run that has been stopped: complete, unless listed
+     * in `lost` (requests an unclean stop -- dead kernel -- never saw complete)                        */
+    std::atomic<uint64_t> done_upto{1};
+    std::atomic<int> any_lost{0};
+    std::mutex lost_mu;
+    std::vector<uint64_t> lost;           /* sorted */
+    bool broken = false;                  /* a CUDA call failed: rebuild everything at the next start */
 };
 
 Engine g_eng;
@@ -96,6 +108,9 @@ inline bool engine_dead(const Engine &e)
 
 void free_engine_memory(Engine &e)
 {
+    /* key hygiene: raw keys sit in ring slots, expanded ones in ktab */
+    if (e.hring) explicit_bzero(e.hring, (size_t)e.R * sizeof(aesoff_host_slot_t));
+    if (e.ktab) cudaMemset(e.ktab, 0, (size_t)(AESOFF_KEY_IDS + e.R) * sizeof(aesoff_key_t));
     if (e.hring) cudaFreeHost(e.hring);
     if (e.hmail) cudaFreeHost(e.hmail);
     if (e.hctl) cudaFreeHost(e.hctl);
@@ -235,6 +250,7 @@ extern "C" void aes_ctx_destroy(aes_ctx_t *ctx)
         /* requests in flight may still name the index: it rests until they must have completed */
         if (ctx->epoch == e.k_epoch.load()) e.id_free.emplace_back(ctx->id, e.next_seq.load());
     }
+    explicit_bzero(ctx, sizeof(*ctx)); /* key hygiene: raw key and round keys do not outlive the context */
     free(ctx);
 }
 
@@ -304,7 +320,8 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
 
     /* ring, mailbox and queues survive a stop/start cycle with the same geometry (a restart then costs
      * one launch, not a dozen allocations) */
-    const bool reuse = e.hring && e.device == device && e.R == o.ring_slots;
+    const bool reuse = e.hring && !e.broken && e.device == device && e.R == o.ring_slots;
+    e.broken = false;
     if (!reuse) free_engine_memory(e);
     e.device = device;
     e.sm_count = sms;
@@ -385,6 +402,13 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
         }
         CPU_RELAX();
     }
+    if (engine_dead(e)) {
+        /* The kernel has already come and gone (ALIVE == 2): the launch was serialised -- a profiler, a
+         * sanitizer or CUDA_LAUNCH_BLOCKING makes the launch call wait for the kernel, which then sits out
+         * its idle timer with nobody able to submit.  A dead engine is not a running one.               */
+        cudaStreamSynchronize(e.stream);
+        return fail(AES_E_STOPPED);
+    }
     e.running.store(1, std::memory_order_release);
     return AES_OK;
 }
@@ -394,15 +418,16 @@ extern "C" int aes_engine_stop(void)
     std::lock_guard<std::mutex> lk(g_lifecycle);
     Engine &e = g_eng;
     if (!e.running.load()) return fail(AES_E_STOPPED);
-    /* no new submissions from here on */
-    e.running.store(2, std::memory_order_release);
+    /* no new submissions from here on; the ones that passed their `running` check finish publishing */
+    e.running.store(2, std::memory_order_seq_cst);
+    while (e.submitters.load(std::memory_order_seq_cst) != 0) CPU_RELAX();
     int rc = AES_OK;
     /* drain: every accepted request completes (unless the kernel died) */
     const uint64_t last = e.next_seq.load();
-    for (uint64_t s = (last > e.first_seq + e.R) ? last - e.R : e.first_seq; s < last; ++s) {
+    const uint64_t lo = (last > e.first_seq + e.R) ? last - e.R : e.first_seq;
+    for (uint64_t s = lo; s < last; ++s) {
         const uint64_t t0 = now_ns();
         while (__atomic_load_n(&e.hmail[(s - 1) & e.Rm], __ATOMIC_ACQUIRE) < s) {
-            /* a producer that claimed s has published it before submit returned, so this ends */
             if (engine_dead(e) || now_ns() - t0 > 60ull * 1000000000ull) {
                 rc = AES_E_STOPPED;
                 break;
@@ -413,7 +438,18 @@ extern "C" int aes_engine_stop(void)
     }
     __atomic_store_n(&e.hctl[AESOFF_CTL_STOP], 1u, __ATOMIC_RELEASE);
     if (cudaStreamSynchronize(e.stream) != cudaSuccess) rc = AES_E_CUDA;
-    if (rc != AES_OK) free_engine_memory(e); /* otherwise kept for the next start */
+    if (rc != AES_OK) {
+        /* unclean stop: the requests the mailbox never saw complete are lost, and aes_poll says so */
+        std::lock_guard<std::mutex> ll(e.lost_mu);
+        for (uint64_t s = lo; s < last; ++s)
+            if (__atomic_load_n(&e.hmail[(s - 1) & e.Rm], __ATOMIC_ACQUIRE) < s) e.lost.push_back(s);
+        if (e.lost.size() > 65536) e.lost.erase(e.lost.begin(), e.lost.end() - 65536);
+        e.any_lost.store(e.lost.empty() ? 0 : 1, std::memory_order_release);
+    }
+    e.done_upto.store(last, std::memory_order_release);
+    /* ring, mailbox and queues are kept for the next start (aes_poll may still be reading the mailbox);
+     * after a CUDA error the next start rebuilds them */
+    if (rc == AES_E_CUDA) e.broken = true;
     e.running.store(0, std::memory_order_release);
     if (rc != AES_OK) return fail(rc);
     return AES_OK;
@@ -466,7 +502,14 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
         fail(rc);
         return 0;
     }
-    if (e.running.load(std::memory_order_acquire) != 1 || engine_dead(e)) {
+    /* counted BEFORE the running check: aes_engine_stop sets running = 2 and then waits for the count to
+     * drop to 0, so a submit either fails here or has published its slot before the drain reads next_seq */
+    struct InFlight {
+        std::atomic<int> &n;
+        explicit InFlight(std::atomic<int> &c) : n(c) { n.fetch_add(1, std::memory_order_seq_cst); }
+        ~InFlight() { n.fetch_sub(1, std::memory_order_seq_cst); }
+    } in_flight(e.submitters);
+    if (e.running.load(std::memory_order_seq_cst) != 1 || engine_dead(e)) {
         fail(AES_E_STOPPED);
         return 0;
     }
@@ -520,10 +563,18 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
     uint32_t icb[4];
     memcpy(icb, nonce, 16);
     uint32_t *w = e.hring[(s - 1) & e.Rm].w;
-    if (kw & AESOFF_KW_RAW) { /* second line first: the dispatcher wants it whenever line one says RAW */
+    /* second line first: the dispatcher wants it whenever line one says RAW.  It is rewritten by EVERY
+     * submit (zeros when the key travels by index): tags are the low 32 bits of the sequence number, and a
+     * raw-key line left over from 2^32 requests ago must never be paired with a fresh first line.        */
+    if (kw & AESOFF_KW_RAW) {
         store_piece(w + 16, ctx->key[0], ctx->key[1], ctx->key[2], tag);
         store_piece(w + 20, ctx->key[3], ctx->key[4], ctx->key[5], tag);
         store_piece(w + 24, ctx->key[6], ctx->key[7], 0u, tag);
+        store_piece(w + 28, 0u, 0u, 0u, tag);
+    } else {
+        store_piece(w + 16, 0u, 0u, 0u, tag);
+        store_piece(w + 20, 0u, 0u, 0u, tag);
+        store_piece(w + 24, 0u, 0u, 0u, tag);
         store_piece(w + 28, 0u, 0u, 0u, tag);
     }
     store_piece(w + 0, icb[0], icb[1], icb[2], tag);
@@ -539,7 +590,15 @@ extern "C" int aes_poll(aes_handle_t h)
 {
     Engine &e = g_eng;
     if (h == 0 || h >= e.next_seq.load(std::memory_order_acquire)) return fail(AES_E_INVAL);
-    if (h < e.first_seq || !e.running.load(std::memory_order_acquire)) return 1; /* a stop drains everything */
+    if (h < e.done_upto.load(std::memory_order_acquire)) {
+        /* a run that has been stopped: a clean stop drained everything, an unclean one lists what it lost */
+        if (e.any_lost.load(std::memory_order_acquire)) {
+            std::lock_guard<std::mutex> lk(e.lost_mu);
+            if (std::binary_search(e.lost.begin(), e.lost.end(), (uint64_t)h)) return fail(AES_E_STOPPED);
+        }
+        return 1;
+    }
+    if (!e.hmail) return fail(AES_E_STOPPED);
     if (__atomic_load_n(&e.hmail[(h - 1) & e.Rm], __ATOMIC_ACQUIRE) >= h) return 1;
     if (engine_dead(e)) {
         /* the exit path of the kernel cannot overtake a completion it already signalled */
@@ -549,15 +608,30 @@ extern "C" int aes_poll(aes_handle_t h)
     return 0;
 }
 
+/* Spins (pause) for the first ~20 us -- the offloads this engine is built for complete in 10 -- then yields the
+ * core between polls, then sleeps in growing steps up to 50 us: a 32-thread executor waiting on
+ * long requests does not burn 32 cores.                                                                       */
 extern "C" int aes_wait(aes_handle_t h, uint64_t timeout_ns)
 {
     const uint64_t t0 = now_ns();
+    uint32_t sleep_ns = 1000;
     for (uint32_t spins = 0;; ++spins) {
         const int r = aes_poll(h);
         if (r == 1) return AES_OK;
         if (r < 0) return r;
-        if ((spins & 63u) == 63u && timeout_ns != UINT64_MAX && now_ns() - t0 > timeout_ns) return fail(AES_E_TIMEOUT);
-        CPU_RELAX();
+        if (spins < 2048u) {
+            if ((spins & 63u) == 63u && timeout_ns != UINT64_MAX && now_ns() - t0 > timeout_ns) return fail(AES_E_TIMEOUT);
+            CPU_RELAX();
+            continue;
+        }
+        if (timeout_ns != UINT64_MAX && now_ns() - t0 > timeout_ns) return fail(AES_E_TIMEOUT);
+        if (spins < 2048u + 256u) {
+            sched_yield();
+        } else {
+            struct timespec ts = {0, (long)sleep_ns};
+            nanosleep(&ts, nullptr);
+            if (sleep_ns < 50000u) sleep_ns *= 2;
+        }
     }
 }
 
@@ -597,6 +671,12 @@ struct LaunchCtx {
     uint32_t *dq_done = nullptr, *dT0 = nullptr;
     cudaEvent_t stage_free = nullptr;
     bool stage_busy = false;
+    /* The device blob (counters, descriptors, keys, tickets) is shared by all calls: a call on another stream
+     * must not overwrite it while the previous call's kernel still reads it.  Every call makes its stream wait
+     * for the previous call's kernel (one event), so calls from any streams are serialised on the device
+     * in call order -- the payload of one launch fills the GPU anyway.                                    */
+    cudaEvent_t kernel_done = nullptr;
+    bool kernel_pending = false;
 };
 LaunchCtx g_lc;
 
@@ -650,12 +730,18 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     if (L.device != device || L.cap_req < R || L.cap_tickets < TM) {
         if (L.stage_busy) cudaEventSynchronize(L.stage_free);
         L.stage_busy = false;
+        if (L.kernel_pending) cudaEventSynchronize(L.kernel_done);
+        L.kernel_pending = false;
         if (L.blob) cudaFree(L.blob);
         if (L.dev_done_seq) cudaFree(L.dev_done_seq);
         if (L.dq_done) cudaFree(L.dq_done);
         if (L.dT0) cudaFree(L.dT0);
-        if (L.stage) cudaFreeHost(L.stage);
+        if (L.stage) {
+            explicit_bzero(L.stage, L.blob_bytes); /* key hygiene: expanded keys were staged here */
+            cudaFreeHost(L.stage);
+        }
         if (!L.stage_free) cudaEventCreateWithFlags(&L.stage_free, cudaEventDisableTiming);
+        if (!L.kernel_done) cudaEventCreateWithFlags(&L.kernel_done, cudaEventDisableTiming);
         L.blob = nullptr;
         L.cap_req = R > L.cap_req ? R : L.cap_req;
         L.cap_tickets = TM > L.cap_tickets ? TM : L.cap_tickets;
@@ -751,7 +837,9 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
 #endif
     const size_t used = off_tk + (size_t)total * sizeof(aesoff_ticket_t);
 
-    bool ok = cudaMemcpyAsync(L.blob, L.stage, used, cudaMemcpyHostToDevice, stream) == cudaSuccess;
+    bool ok = true;
+    if (L.kernel_pending) ok = cudaStreamWaitEvent(stream, L.kernel_done, 0) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(L.blob, L.stage, used, cudaMemcpyHostToDevice, stream) == cudaSuccess;
     ok = ok && cudaEventRecord(L.stage_free, stream) == cudaSuccess;
     L.stage_busy = true;
     if (!ok) {
@@ -781,6 +869,7 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     if (ctas > (uint64_t)sms) ctas = (uint64_t)sms;
     if (ctas == 0) ctas = 1;
     if (aesoff_launch_engine(&p, (int)ctas, stream) != 0) return fail(AES_E_CUDA);
+    L.kernel_pending = cudaEventRecord(L.kernel_done, stream) == cudaSuccess;
     g_kernel_launches.fetch_add(1);
     return AES_OK;
 }

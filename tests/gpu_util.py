@@ -50,3 +50,17 @@ def first_mismatch(got: np.ndarray, want: bytes) -> int:
         return -2
     ne = np.nonzero(got != w)[0]
     return int(ne[0]) if ne.size else -1
+
+
+def verify_requests(w, idxs, out_of, workers: int | None = None):
+    """Every byte of requests `idxs` of workload `w` against the oracle, on a thread pool (the payload is
+    regenerated from the seed, the oracle call releases the GIL).  out_of(i) -> uint8 ndarray of request i's
+    output.  Returns [(request, first mismatching byte or -2 for a length mismatch)], empty when all match."""
+    workers = workers or max(1, len(os.sched_getaffinity(0)))
+
+    def one(i):
+        want = o.ctr(w.key_of(i), w.icb_of(i), w.payload(i))
+        return i, first_mismatch(out_of(i), want)
+
+    with cf.ThreadPoolExecutor(workers) as ex:
+        return [(i, b) for i, b in ex.map(one, idxs) if b != -1]
