@@ -331,3 +331,76 @@ void oracle_ctr(const uint8_t *rk, int nr, const uint8_t icb[16],
 {
     oracle_ctr_at(rk, nr, icb, 0, src, dst, len);
 }
+
+/* ------------------------------------------------------------------------ */
+/* SP 800-38A sec. 6.1 ECB mode and sec. 6.2 CBC mode, whole blocks only (the   */
+/* standard defines both on a sequence of complete blocks; padding is the       */
+/* caller's business, sec. 5.2 / appendix A).  DESIGN.md reading R13: the paper */
+/* "performs AES" without naming a mode; CTR is the mode the     */
+/* benchmark fixes, ECB and CBC decryption are the other two modes in which     */
+/* every block can be computed independently.         */
+/* ------------------------------------------------------------------------ */
+
+/* ECB encryption: C_j = CIPH_K(P_j), j = 1..n (sec. 6.1).                    */
+void oracle_ecb_encrypt(const uint8_t *rk, int nr, const uint8_t *src, uint8_t *dst, size_t nblocks)
+{
+    size_t j;
+    for (j = 0; j < nblocks; j++) {
+        uint8_t P[16], C[16];
+        memcpy(P, src + 16 * j, 16);
+        oracle_encrypt_block(rk, nr, P, C);
+        memcpy(dst + 16 * j, C, 16);
+    }
+}
+
+/* ECB decryption: P_j = CIPH^-1_K(C_j), j = 1..n (sec. 6.1).                 */
+void oracle_ecb_decrypt(const uint8_t *rk, int nr, const uint8_t *src, uint8_t *dst, size_t nblocks)
+{
+    size_t j;
+    for (j = 0; j < nblocks; j++) {
+        uint8_t C[16], P[16];
+        memcpy(C, src + 16 * j, 16);
+        oracle_decrypt_block(rk, nr, C, P);
+        memcpy(dst + 16 * j, P, 16);
+    }
+}
+
+/* CBC encryption: C_1 = CIPH_K(P_1 xor IV); C_j = CIPH_K(P_j xor C_{j-1}), j = 2..n
+ * (sec. 6.2).  Sequential by definition; here so that tests have ciphertexts to
+ * decrypt and a round trip to check -- the GPU path only decrypts.            */
+void oracle_cbc_encrypt(const uint8_t *rk, int nr, const uint8_t iv[16], const uint8_t *src, uint8_t *dst,
+                        size_t nblocks)
+{
+    uint8_t prev[16];
+    size_t j;
+    int i;
+    memcpy(prev, iv, 16);                        /* "C_0" = IV                 */
+    for (j = 0; j < nblocks; j++) {
+        uint8_t X[16], C[16];
+        for (i = 0; i < 16; i++)
+            X[i] = (uint8_t)(src[16 * j + i] ^ prev[i]);
+        oracle_encrypt_block(rk, nr, X, C);
+        memcpy(dst + 16 * j, C, 16);
+        memcpy(prev, C, 16);
+    }
+}
+
+/* CBC decryption: P_1 = CIPH^-1_K(C_1) xor IV; P_j = CIPH^-1_K(C_j) xor C_{j-1},
+ * j = 2..n (sec. 6.2).  dst may equal src (the previous ciphertext block is
+ * kept in a local copy).                                                       */
+void oracle_cbc_decrypt(const uint8_t *rk, int nr, const uint8_t iv[16], const uint8_t *src, uint8_t *dst,
+                        size_t nblocks)
+{
+    uint8_t prev[16];
+    size_t j;
+    int i;
+    memcpy(prev, iv, 16);
+    for (j = 0; j < nblocks; j++) {
+        uint8_t C[16], X[16];
+        memcpy(C, src + 16 * j, 16);
+        oracle_decrypt_block(rk, nr, C, X);
+        for (i = 0; i < 16; i++)
+            dst[16 * j + i] = (uint8_t)(X[i] ^ prev[i]);
+        memcpy(prev, C, 16);
+    }
+}

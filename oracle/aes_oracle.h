@@ -15,6 +15,7 @@
  *   - KeyExpansion                                         FIPS-197 sec. 5.2
  *   - Cipher / InvCipher                                   FIPS-197 sec. 5.1 / 5.3
  *   - CTR with a 128-bit big-endian incrementing function  SP 800-38A sec. 6.5, B.1
+ *   - ECB and CBC on whole blocks          SP 800-38A sec. 6.1, 6.2
  *
  * Pins: every function below is pinned by tests/test_oracle_*.py (-m "not gpu")
  * against the standards' printed vectors (tests/golden/), OpenSSL libcrypto,
@@ -74,6 +75,21 @@ void oracle_ctr_at(const uint8_t *rk, int nr, const uint8_t icb[16], uint64_t bl
 
 /* icb + add (mod 2^128, big-endian) -> out.  Exposed so tests can pin it.   */
 void oracle_ctr_add(const uint8_t icb[16], uint64_t add, uint8_t out[16]);
+
+/* ---- ECB and CBC (SP 800-38A sec. 6.1, 6.2) -------------------------------
+ * Whole blocks only: nblocks x 16 bytes, no padding (the standard defines both
+ * modes on complete blocks).  ECB: C_j = CIPH_K(P_j) / P_j = CIPH^-1_K(C_j).
+ * CBC: C_1 = CIPH_K(P_1 xor IV), C_j = CIPH_K(P_j xor C_{j-1});
+ *      P_1 = CIPH^-1_K(C_1) xor IV, P_j = CIPH^-1_K(C_j) xor C_{j-1}.
+ * dst may equal src in all four.  The GPU path has ECB both ways and CBC
+ * decryption (every block independent); CBC encryption is sequential by
+ * definition and is here for the tests' round trips.                          */
+void oracle_ecb_encrypt(const uint8_t *rk, int nr, const uint8_t *src, uint8_t *dst, size_t nblocks);
+void oracle_ecb_decrypt(const uint8_t *rk, int nr, const uint8_t *src, uint8_t *dst, size_t nblocks);
+void oracle_cbc_encrypt(const uint8_t *rk, int nr, const uint8_t iv[16], const uint8_t *src, uint8_t *dst,
+                        size_t nblocks);
+void oracle_cbc_decrypt(const uint8_t *rk, int nr, const uint8_t iv[16], const uint8_t *src, uint8_t *dst,
+                        size_t nblocks);
 
 #ifdef __cplusplus
 }

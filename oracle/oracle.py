@@ -71,6 +71,10 @@ def lib() -> ctypes.CDLL:
                 ("oracle_ctr", None, [ctypes.c_void_p, i32, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, sz]),
                 ("oracle_ctr_at", None, [ctypes.c_void_p, i32, ctypes.c_void_p, u64, ctypes.c_void_p, ctypes.c_void_p, sz]),
                 ("oracle_ctr_add", None, [ctypes.c_void_p, u64, ctypes.c_void_p]),
+                ("oracle_ecb_encrypt", None, [ctypes.c_void_p, i32, ctypes.c_void_p, ctypes.c_void_p, sz]),
+                ("oracle_ecb_decrypt", None, [ctypes.c_void_p, i32, ctypes.c_void_p, ctypes.c_void_p, sz]),
+                ("oracle_cbc_encrypt", None, [ctypes.c_void_p, i32, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, sz]),
+                ("oracle_cbc_decrypt", None, [ctypes.c_void_p, i32, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, sz]),
             ]:
                 fn = getattr(L, name)
                 fn.restype = res
@@ -148,3 +152,25 @@ def ctr_into(key: bytes, icb: bytes, src_addr: int, dst_addr: int, n: int, block
     """Pointer form for the timed cpu_baseline leg (no copies; releases the GIL)."""
     rk, nr = key_expand(key)
     lib().oracle_ctr_at(rk, nr, bytes(icb), block_offset, src_addr, dst_addr, n)
+
+
+def _blocks(name: str, key: bytes, data, iv: bytes | None = None) -> bytes:
+    rk, nr = key_expand(key)
+    mv = memoryview(data).cast("B")
+    n = mv.nbytes
+    if n % 16:
+        raise ValueError("ECB/CBC take whole 16-byte blocks (SP 800-38A sec. 6.1, 6.2)")
+    out = ctypes.create_string_buffer(max(n, 1))
+    src = (ctypes.c_uint8 * n).from_buffer_copy(mv) if n else None
+    if iv is None:
+        getattr(lib(), name)(rk, nr, src, out, n // 16)
+    else:
+        assert len(iv) == 16
+        getattr(lib(), name)(rk, nr, bytes(iv), src, out, n // 16)
+    return out.raw[:n]
+
+
+def ecb_encrypt(key: bytes, data) -> bytes: return _blocks("oracle_ecb_encrypt", key, data)
+def ecb_decrypt(key: bytes, data) -> bytes: return _blocks("oracle_ecb_decrypt", key, data)
+def cbc_encrypt(key: bytes, iv: bytes, data) -> bytes: return _blocks("oracle_cbc_encrypt", key, data, iv)
+def cbc_decrypt(key: bytes, iv: bytes, data) -> bytes: return _blocks("oracle_cbc_decrypt", key, data, iv)
