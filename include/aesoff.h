@@ -66,7 +66,7 @@ typedef uint64_t       aes_handle_t;  /* submission sequence number, from 1; 0 =
 
 /* ---- engine life cycle (step a0 of the path) -------------------------------
  * The engine is: a pinned, host-mapped descriptor ring; ONE persistent sm_100a
- * kernel (a dispatcher warp that polls the ring over PCIe, and per SM one
+ * kernel (dispatcher warps that poll the ring over PCIe, and per SM one
  * service warp plus 16 worker warps around the AES tables in shared memory);
  * and a host-mapped completion
  * mailbox.  A request therefore never pays a kernel launch (the paper's 4 KiB
@@ -75,18 +75,21 @@ typedef uint64_t       aes_handle_t;  /* submission sequence number, from 1; 0 =
 typedef struct aes_engine_opts {
     uint32_t ring_slots;      /* descriptor ring depth = max requests in flight; power of
                                  two in [64, 4096]; 0 = default 2048                      */
-    uint32_t chunk_rows;      /* work-item size in 4 KiB rows (256 counter values each);
-                                 1..64; 0 = default 4 (16 KiB per worker-group item)      */
+    uint32_t chunk_rows;      /* work-item size in 4 KiB rows (256 counter values each): a power
+                                 of two, 1..64; 0 = default 4 (16 KiB per worker-group item) */
     uint32_t n_ctas;          /* persistent CTAs; 0 = one per SM                          */
     uint32_t idle_exit_ms;    /* the kernel exits by itself (engine becomes STOPPED) after
                                  this long with no request; 0 = never                     */
     uint32_t fine_rows;       /* latency modes: a request of at most this many 4 KiB rows may
                                  be cut into units smaller than a row -- 1/8 row (32 blocks per
-                                 warp) when it finds the GPU idle, half a row when the queue is
-                                 short -- so that it spreads over many warps; requests up to 16
-                                 rows are always cut into 1/8 rows.  0 = default 2048 (8 MiB),
+                                 warp) at the front of an idle GPU's queue, half a row while the
+                                 queue is short and at the end of a long lone request -- so that
+                                 it spreads over many warps.  0 = default (any size),
                                  AES_FINE_ROWS_OFF = whole rows only                        */
-    uint32_t reserved[3];     /* must be 0                                                */
+    uint32_t n_dispatchers;   /* warps that poll the ring and cut requests into work items, one
+                                 each on the first CTAs; consecutive batches of 32 sequence
+                                 numbers go round them.  1..8; 0 = default 2               */
+    uint32_t reserved[2];     /* must be 0                                                */
 } aes_engine_opts_t;
 
 /* Starts the engine on CUDA device `device`.  opts == NULL means all defaults.
@@ -124,7 +127,7 @@ typedef struct aes_engine_info {
     uint32_t ring_slots;
     uint32_t chunk_rows;
     uint32_t smem_bytes_per_cta;
-    uint32_t reserved0;
+    uint32_t n_dispatchers;      /* dispatcher warps of the running engine            */
     uint64_t submitted;          /* requests accepted so far                         */
     uint64_t completed;          /* requests whose completion the host has observed
                                     through aes_poll/aes_wait, lower bound            */
@@ -170,7 +173,7 @@ int aes_ctx_round_keys(const aes_ctx_t *ctx, uint8_t *out);
  *          completion.
  *   dst    same kinds of memory, 16-byte aligned, len bytes.  dst == src (in
  *          place) is allowed; any other overlap is AES_E_OVERLAP.
- *   len    any value >= 0; len == 0 completes without touching memory.
+ *   len    any value >= 0 and < 2^36 (64 GiB); len == 0 completes without touching memory.
  *
  * Never blocks.  Returns the handle (>= 1), or 0 with aes_last_error() in
  * {AES_E_INVAL, AES_E_ALIGN, AES_E_OVERLAP, AES_E_AGAIN (ring full), AES_E_STOPPED}.

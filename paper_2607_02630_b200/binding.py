@@ -41,14 +41,15 @@ class AesOffError(RuntimeError):
 
 class aes_engine_opts_t(ctypes.Structure):
     _fields_ = [("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32), ("n_ctas", ctypes.c_uint32),
-                ("idle_exit_ms", ctypes.c_uint32), ("fine_rows", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 3)]
+                ("idle_exit_ms", ctypes.c_uint32), ("fine_rows", ctypes.c_uint32), ("n_dispatchers", ctypes.c_uint32),
+                ("reserved", ctypes.c_uint32 * 2)]
 
 
 class aes_engine_info_t(ctypes.Structure):
     _fields_ = [("running", ctypes.c_int32), ("device", ctypes.c_int32), ("sm_count", ctypes.c_int32),
                 ("n_ctas", ctypes.c_int32), ("threads_per_cta", ctypes.c_int32), ("worker_warps_per_cta", ctypes.c_int32),
                 ("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32),
-                ("smem_bytes_per_cta", ctypes.c_uint32), ("reserved0", ctypes.c_uint32),
+                ("smem_bytes_per_cta", ctypes.c_uint32), ("n_dispatchers", ctypes.c_uint32),
                 ("submitted", ctypes.c_uint64), ("completed", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64),
                 ("cut_eighths", ctypes.c_uint64), ("cut_halves", ctypes.c_uint64), ("cut_rows", ctypes.c_uint64)]
 
@@ -126,8 +127,8 @@ def _check(rc: int, where: str) -> None:
 
 # ---- engine ---------------------------------------------------------------------------------
 def aes_engine_start(device: int = 0, ring_slots: int = 0, chunk_rows: int = 0, n_ctas: int = 0,
-                     idle_exit_ms: int = 0, fine_rows: int = 0) -> None:
-    o = aes_engine_opts_t(ring_slots, chunk_rows, n_ctas, idle_exit_ms, fine_rows)
+                     idle_exit_ms: int = 0, fine_rows: int = 0, n_dispatchers: int = 0) -> None:
+    o = aes_engine_opts_t(ring_slots, chunk_rows, n_ctas, idle_exit_ms, fine_rows, n_dispatchers)
     _check(_lib.aes_engine_start(device, ctypes.byref(o)), "aes_engine_start")
 
 
@@ -138,7 +139,7 @@ def aes_engine_stop() -> None:
 def aes_engine_info() -> dict:
     info = aes_engine_info_t()
     _check(_lib.aes_engine_info(ctypes.byref(info)), "aes_engine_info")
-    return {k: getattr(info, k) for k, _ in aes_engine_info_t._fields_ if k != "reserved0"}
+    return {k: getattr(info, k) for k, _ in aes_engine_info_t._fields_}
 
 
 # ---- contexts ---------------------------------------------------------------------------------

@@ -7,10 +7,12 @@
 #include "aesoff_shared.h"
 
 /* How a context's key reaches the device (aesoff_runtime.cpp, aes_ctr_submit):
- *   first submit        the raw key rides in the descriptor, the dispatcher expands it (one-shot
- *                       contexts, BASELINE.json configs[3], never own device state)
- *   second submit       as above, and the dispatcher also stores the expanded key at ktab[id]
- *   later submits       the descriptor only names ktab[id]                                       */
+ *   first submit        the raw key rides in the descriptor, the dispatcher that takes the request
+ *                       expands it (one-shot contexts, BASELINE.json configs[3], never own device state)
+ *   second submit       as above, and that dispatcher also stores the expanded key at ktab[id]
+ *   until that request has COMPLETED (mailbox)   raw key again, nothing stored: several dispatcher warps
+ *                       take requests side by side, so "submitted earlier" does not mean "expanded earlier"
+ *   afterwards          the descriptor only names ktab[id]                                       */
 #define AESOFF_CTX_FRESH      0u
 #define AESOFF_CTX_SEEN       1u
 #define AESOFF_CTX_INSTALLING 2u
@@ -24,6 +26,7 @@ struct aes_ctx {
     uint32_t state;  /* AESOFF_CTX_*, accessed atomically */
     uint32_t id;     /* ktab index once state >= INSTALLING */
     uint64_t epoch;  /* ktab generation the id belongs to */
+    uint64_t install_seq; /* sequence number of the request that installs the key (0 = not claimed yet) */
     uint32_t rk_ready; /* rk[] has been filled (lazily: the engine path expands keys on the device) */
 };
 

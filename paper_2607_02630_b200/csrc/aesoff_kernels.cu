@@ -63,8 +63,9 @@ struct __align__(16) CtaCtl {
     uint32_t busy[AESOFF_SLOTS];  /* 0 free, 1 filled and not yet completed                      */
     uint32_t exit_flag;
     uint32_t pad[3];
-    /* dispatcher (CTA 0): the descriptors of one poll, as read from the host ring */
-    uint32_t stage[32][AESOFF_STAGE_STRIDE];
+    /* dispatcher CTAs: two landing areas for polls of the host ring (one is looked at while the next poll
+     * flies): 32 descriptors as read from the ring, and a 33rd row for the control words that come with them */
+    uint32_t stage[2][33][AESOFF_STAGE_STRIDE];
 };
 constexpr uint32_t CTRL_BYTES = sizeof(CtaCtl);
 constexpr uint32_t CLAIM_EXIT = 0xffffffffu;
@@ -90,12 +91,6 @@ __device__ __forceinline__ void st_release_gpu(unsigned long long *p, unsigned l
 {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
-__device__ __forceinline__ uint32_t ld_volatile_u32(const volatile uint32_t *p)
-{
-    uint32_t v;
-    asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
 __device__ __forceinline__ uint4 ld_volatile_v4(const void *p)
 {
     uint4 v;
@@ -105,6 +100,16 @@ __device__ __forceinline__ uint4 ld_volatile_v4(const void *p)
                  : "memory");
     return v;
 }
+/* 16 bytes global (or host-mapped) memory -> shared memory without a register in between: a poll in flight
+ * holds no destination registers and no scoreboard that an LDS or SHFL of the code running under it could
+ * end up waiting on (L2 only: mapped host memory is not cached on the GPU, every copy goes to the host) */
+__device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc)
+                 : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ unsigned long long globaltimer_ns()
 {
     unsigned long long t;
@@ -181,8 +186,8 @@ __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase,
         if (got == CLAIM_EXIT) break;
 #ifdef AESOFF_DEBUG
         if (lane == 0 && first) {
-            atomicMin(reinterpret_cast<unsigned long long *>(P.counters) + 20 + 3, globaltimer_ns()); /* first unit claimed anywhere */
-            atomicMax(reinterpret_cast<unsigned long long *>(P.counters) + 20 + 4, globaltimer_ns()); /* last warp gets its first unit */
+            atomicMin(reinterpret_cast<unsigned long long *>(P.counters) + AESOFF_CNT_DEBUG + 3, globaltimer_ns()); /* first unit claimed anywhere */
+            atomicMax(reinterpret_cast<unsigned long long *>(P.counters) + AESOFF_CNT_DEBUG + 4, globaltimer_ns()); /* last warp gets its first unit */
         }
         first = false;
 #endif
@@ -408,110 +413,192 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
 }
 
 /* ------------------------------------------------------------------------------------------ */
-/* dispatcher warp (persistent mode, CTA 0): host ring -> device queue + tickets  (a3)         */
+/* dispatcher warps (persistent mode, warp 17 of CTAs 0 .. n_disp-1): host ring -> tickets (a3) */
 /* ------------------------------------------------------------------------------------------ */
-/* One iteration = ONE PCIe round trip: the warp reads the next 8 (quiet) or 32 (busy) ring slots,
- * 128 B each, as 16-byte pieces that validate themselves (aesoff_shared.h), so there is no
- * flag-then-body dependency.  Everything after that is on-chip or L2: geometry, key expansion
- * for raw keys, descriptor and ticket stores, one release of the published count.             */
-__device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase, uint32_t lane)
+/* Sequence numbers are dealt out in batches of 32: batch b = [first_seq + 32 b, +32) belongs to dispatcher
+ * b % n_disp, lane k of that warp to request k of the batch.  A dispatcher reads its batch's ring slots
+ * (8 when quiet, all 32 when busy; 128 B each, as 16-byte pieces that validate themselves, so there is no
+ * flag-then-body dependency) in ONE PCIe round trip, and takes the ready prefix.
+ *
+ * Tickets are numbered in sequence order, so the dispatchers pass a token along: one 16-byte word
+ * {tickets published, next sequence number to dispatch} in device memory (AESOFF_CNT_CHAIN).  A dispatcher
+ * whose next request is chain.next holds the token: it sizes units and chunks by the load it sees, adds
+ * its ticket count, stores the word for the next one -- a fraction of a microsecond -- and only then does
+ * the long part (key expansion for raw keys, descriptors, tickets) beside the other dispatchers.  The word
+ * is read with every poll, so a lone request never waits for it.                                         */
+__device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase, uint32_t lane, uint32_t d)
 {
-    unsigned long long *g_idle = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_IDLE);
     unsigned long long *g_published = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_PUBLISHED);
     unsigned long long *g_stop = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_STOP);
+    unsigned long long *g_quit = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_QUIT);
+    uint4 *g_chain = reinterpret_cast<uint4 *>(P.counters + AESOFF_CNT_CHAIN);
     const uint32_t Rm = P.R - 1;
-    unsigned long long next_seq = P.first_seq; /* next sequence number to take from the ring   */
-    unsigned long long published = 0;          /* tickets published so far                     */
+    const uint32_t K = P.n_disp;
+    unsigned long long b_seq = P.first_seq + (unsigned long long)AESOFF_BATCH * d; /* first request of my batch   */
+    uint32_t pos = 0;                          /* requests of it already dispatched            */
+    bool have_token = false;                   /* chain.next == b_seq + pos, and I know it     */
+    unsigned long long my_pub = 0;             /* chain.published while I hold the token       */
     unsigned long long oldest = P.first_seq;   /* every seq below this is known to be complete */
     unsigned long long base = 0;               /* first ticket of request `oldest` at the last scan */
-    unsigned long long last_activity = globaltimer_ns();
+    unsigned long long last_activity = globaltimer_ns(), seen_next = 0;
     uint32_t wide = 0;                         /* 0: poll 8 slots, 1: poll 32                  */
     uint32_t n_eighths = 0, n_halves = 0, n_rows = 0;
     bool stats_dirty = false;
+#ifdef AESOFF_DISP_STATS
+    uint32_t dbg_takes = 0, dbg_reqs = 0, dbg_empty = 0;
+    unsigned long long dbg_wait = 0, dbg_work = 0;
+#endif
 
-    if (lane == 0) P.hctl[AESOFF_CTL_ALIVE] = 1;
+    if (lane == 0 && d == 0) P.hctl[AESOFF_CTL_ALIVE] = 1;
 
-    /* One poll = the next 8 (quiet) or 32 (busy) ring slots as 16-byte pieces, plus the stop word and two
-     * device counters.  piece g = 32 j + lane: slot g / 8 after the poll's first sequence number, piece g % 8.
-     * A poll is issued as soon as the previous one has been looked at, i.e. BEFORE that batch is processed:
-     * the PCIe round trip of the next batch runs under the on-chip work of this one.                       */
-    uint4 pc[8];
-    uint32_t p_stop = 0, p_nload = 2u;
-    unsigned long long p_idle = 0, p_reserved = 0;
-#define ISSUE_POLL(seq0)                                                                                     \
+    /* One poll = ring slots of my batch as 16-byte pieces (piece g = 32 j + lane: slot q + g / 8 of the batch,
+     * piece g % 8), plus the host's control words and three device words: the token, {tickets reserved, published}
+     * and {idle CTAs, quit}.  All of it is copied asynchronously (cp.async) into the landing area the warp is NOT
+     * looking at, and a poll is issued as soon as the previous one has been looked at, i.e. BEFORE that batch is
+     * processed: the PCIe round trip of the next one runs under the on-chip work of this one.  (The polls used to
+     * live in 32 registers; whenever ptxas let an LDS of the processing code share a scoreboard with them, that
+     * LDS waited out the PCIe round trip: +1.6 us on every request, found with a time stamp.)                */
+    uint32_t cur = 0; /* landing area being looked at */
+#define AUX_CTL   0   /* row 32 of a landing area: words 0..3 host control words (0 = stop) */
+#define AUX_CHAIN 4   /*   4..7   the token                                                  */
+#define AUX_TKT   8   /*   8..11  {tickets reserved, tickets published}                      */
+#define AUX_IDLE  12  /*   12..15 {idle CTAs, quit, long queue}                              */
+#define ISSUE_POLL(bseq, q, ring)                                                                            \
     do {                                                                                                     \
-        p_nload = wide ? 8u : 2u;                                                                            \
+        uint32_t(*land_)[AESOFF_STAGE_STRIDE] = c->stage[cur ^ 1u];                                          \
+        const uint32_t nload_ = !(ring) ? 0u : wide ? 8u : 2u;                                               \
+        const uint32_t q_ = wide ? 0u : (q);                                                                 \
         _Pragma("unroll") for (uint32_t j = 0; j < 8; ++j)                                                  \
         {                                                                                                    \
-            pc[j] = make_uint4(0, 0, 0, 0);                                                                  \
-            if (j < p_nload) {                                                                               \
-                const uint32_t k_ = j * 4u + (lane >> 3);                                                    \
-                const uint32_t sl_ = (uint32_t)(((seq0) + k_ - 1) & Rm);                                     \
-                pc[j] = ld_volatile_v4(reinterpret_cast<const uint8_t *>(P.hring + sl_) + 16u * (lane & 7u)); \
+            const uint32_t k_ = q_ + j * 4u + (lane >> 3);                                                   \
+            if (j < nload_ && k_ < AESOFF_BATCH) {                                                           \
+                const uint32_t sl_ = (uint32_t)(((bseq) + k_ - 1) & Rm);                                     \
+                cp_async16(&land_[k_][4u * (lane & 7u)], reinterpret_cast<const uint8_t *>(P.hring + sl_) + 16u * (lane & 7u)); \
             }                                                                                                \
         }                                                                                                    \
         if (lane == 0) {                                                                                     \
-            p_stop = ld_volatile_u32(P.hctl + AESOFF_CTL_STOP);                                              \
-            p_idle = *reinterpret_cast<volatile unsigned long long *>(g_idle);                               \
-            p_reserved = *reinterpret_cast<volatile unsigned long long *>(P.counters + AESOFF_CNT_TICKET);   \
+            if (ring)                                                                                        \
+                cp_async16(&land_[32][AUX_CTL], const_cast<const uint32_t *>(P.hctl));                       \
+            else                                                                                             \
+                land_[32][AUX_CTL + AESOFF_CTL_STOP] = 0u;                                                   \
+        } else if (lane < 4) {                                                                               \
+            cp_async16(&land_[32][4u * lane], P.counters + (lane == 1 ? AESOFF_CNT_CHAIN : lane == 2 ? AESOFF_CNT_TICKET : AESOFF_CNT_IDLE)); \
         }                                                                                                    \
+        cp_async_commit();                                                                                   \
     } while (0)
-    bool repoll = true; /* the poll in flight (if any) does not start at next_seq */
+    bool repoll = true; /* no poll in flight for (b_seq, pos) */
+    /* Only the dispatcher that holds the token can take requests now; what the others read is a prefetch.  Polls
+     * of several warps queue up behind one another on PCIe (four of them polling flat out added 4 us to a lone
+     * request), so: the holder polls continuously; the others only watch the token -- unless the holder has
+     * found a long queue (eight or more requests ready at once: it says so in a device word), in which case
+     * the dispatchers whose batch comes next or next but one read their slots ahead of the token.            */
+    unsigned long long token_at = (K == 1u) ? b_seq : 0ull; /* chain.next as last seen */
+    bool queue_long = false;     /* the holder's last word on it */
 
     for (;;) {
         /* ---- phase 1: the PCIe round trip ---------------------------------------------------- */
-        if (repoll) ISSUE_POLL(next_seq);
+        if (repoll) {
+            const bool holder = have_token || token_at == b_seq + pos;
+            const bool near = holder || (queue_long && token_at + 2ull * AESOFF_BATCH >= b_seq);
+            if (!holder) __nanosleep(queue_long ? 400u : 3000u); /* device words only: no PCIe read (ISSUE_POLL) */
+            ISSUE_POLL(b_seq, pos, near);
+        }
         repoll = false;
-        const uint32_t nload = p_nload;
-        uint32_t stop = p_stop;
-        unsigned long long idle = p_idle, reserved = p_reserved;
-#pragma unroll
-        for (uint32_t j = 0; j < 8; ++j) {
-            if (j < nload) {
-                const uint32_t k = j * 4u + (lane >> 3);
-                *reinterpret_cast<uint4 *>(&c->stage[k][4u * (lane & 7u)]) = pc[j];
-            }
-        }
+        cp_async_wait_all();
+        cur ^= 1u;
         __syncwarp();
-        /* lane k looks at slot k of the poll */
-        const unsigned long long s = next_seq + lane;
+#ifdef AESOFF_DISP_STATS
+        const unsigned long long dbg_t0 = globaltimer_ns(); /* the poll has landed */
+#endif
+        /* lane k looks at request k of the batch (rows outside this poll hold older pieces: their tags
+         * either still match, from an earlier poll of this batch, or belong to another batch) */
+        const unsigned long long s = b_seq + lane;
         const uint32_t slot = (uint32_t)((s - 1) & Rm);
-        const uint32_t *sw = c->stage[lane];
+        const uint32_t *sw = c->stage[cur][lane];
+        const uint32_t *ax = c->stage[cur][32];
         const uint32_t tag = (uint32_t)s;
-        uint32_t kw = 0;
-        bool valid = false;
-        if (lane < nload * 4u) {
-            kw = sw[AESOFF_PW_INDEX(AESOFF_PW_KEY)];
-            valid = sw[3] == tag && sw[7] == tag && sw[11] == tag && sw[15] == tag;
-            if (valid && (kw & AESOFF_KW_RAW))
-                valid = sw[19] == tag && sw[23] == tag && sw[27] == tag && sw[31] == tag;
-        }
-        const uint32_t vmask = __ballot_sync(0xffffffffu, valid);
-        uint32_t n = (vmask == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~vmask) - 1); /* length of the ready prefix */
-        stop = __shfl_sync(0xffffffffu, stop, 0);
-        idle = __shfl_sync(0xffffffffu, idle, 0);
-        reserved = __shfl_sync(0xffffffffu, reserved, 0);
+        uint32_t kw = sw[AESOFF_PW_INDEX(AESOFF_PW_KEY)];
+        bool valid = lane >= pos && sw[3] == tag && sw[7] == tag && sw[11] == tag && sw[15] == tag;
+        if (valid && (kw & AESOFF_KW_RAW)) valid = sw[19] == tag && sw[23] == tag && sw[27] == tag && sw[31] == tag;
+        const uint32_t vrun = ~(__ballot_sync(0xffffffffu, valid) >> pos); /* bit i: request pos + i is not ready */
+        uint32_t n = vrun ? (uint32_t)(__ffs(vrun) - 1) : 32u;           /* length of the ready run from pos */
+        if (n > 32u - pos) n = 32u - pos;
+        const uint32_t stop = ax[AUX_CTL + AESOFF_CTL_STOP];
+        unsigned long long chain_pub = ((unsigned long long)ax[AUX_CHAIN + 1] << 32) | ax[AUX_CHAIN];
+        unsigned long long chain_next = ((unsigned long long)ax[AUX_CHAIN + 3] << 32) | ax[AUX_CHAIN + 2];
+        const unsigned long long reserved = ((unsigned long long)ax[AUX_TKT + 1] << 32) | ax[AUX_TKT];
+        const unsigned long long idle = ((unsigned long long)ax[AUX_IDLE + 1] << 32) | ax[AUX_IDLE];
+        const uint32_t quit_word = ax[AUX_IDLE + 2];
+        queue_long = ax[AUX_IDLE + 3] != 0u;
+        token_at = chain_next;
         wide = (n >= 8u) ? 1u : 0u;
         const uint32_t n_seen = n;
-        if (n != 0) ISSUE_POLL(next_seq + n); /* the staged copy of this poll is in shared memory: pc[] is free */
+#ifdef AESOFF_EARLY_PREFETCH
+        if (n != 0) { /* the next poll lands in the other area */
+            if (pos + n == 32u)
+                ISSUE_POLL(b_seq + (unsigned long long)AESOFF_BATCH * K, 0u, true);
+            else
+                ISSUE_POLL(b_seq, pos + n, true);
+        }
+#endif
         if (n == 0) {
             repoll = true;
+            if (queue_long && (have_token || chain_next == b_seq + pos)) { /* the queue has run dry: the others stop reading ahead */
+                queue_long = false;
+                if (lane == 0) *(reinterpret_cast<volatile uint32_t *>(g_quit) + 1) = 0u;
+            }
+#ifdef AESOFF_DISP_STATS
+            ++dbg_empty;
+#endif
             if (stats_dirty) {
                 /* not on a request's way: a PCIe write in flight would hold up the next fence */
                 if (lane == 0) {
-                    P.hctl[AESOFF_CTL_CUT_EIGHTHS] = n_eighths;
-                    P.hctl[AESOFF_CTL_CUT_HALVES] = n_halves;
-                    P.hctl[AESOFF_CTL_CUT_ROWS] = n_rows;
+                    volatile uint32_t *st = P.hctl + AESOFF_CTL_STATS + AESOFF_CTL_STAT_WORDS * d;
+                    st[AESOFF_CTL_CUT_EIGHTHS] = n_eighths;
+                    st[AESOFF_CTL_CUT_HALVES] = n_halves;
+                    st[AESOFF_CTL_CUT_ROWS] = n_rows;
+#ifdef AESOFF_DISP_STATS
+                    st[AESOFF_CTL_DBG_TAKES] = dbg_takes;
+                    st[AESOFF_CTL_DBG_REQS] = dbg_reqs;
+                    st[AESOFF_CTL_DBG_WAIT] = (uint32_t)(dbg_wait >> 6);
+                    st[AESOFF_CTL_DBG_WORK] = (uint32_t)(dbg_work >> 6);
+                    st[AESOFF_CTL_DBG_EMPTY] = dbg_empty;
+#endif
                 }
                 stats_dirty = false;
             }
-            bool quit = stop != 0;
-            if (!quit && P.idle_exit_ms) {
+            bool quit = stop != 0 || quit_word != 0;
+            if (!quit && d == 0 && P.idle_exit_ms) {
+                /* the idle timer is dispatcher 0's: it runs while no dispatcher takes anything, and fires only
+                 * when everything that was accepted has completed */
                 const unsigned long long now = globaltimer_ns();
-                if (now - last_activity > (unsigned long long)P.idle_exit_ms * 1000000ull) quit = true;
+                if (chain_next != seen_next) {
+                    seen_next = chain_next;
+                    last_activity = now;
+                } else if (now - last_activity > (unsigned long long)P.idle_exit_ms * 1000000ull) {
+                    if (chain_next > oldest + P.R) oldest = chain_next - P.R;
+                    for (;;) {
+                        const unsigned long long q = oldest + lane;
+                        bool fin = false;
+                        if (q < chain_next)
+                            fin = *reinterpret_cast<volatile uint64_t *>(P.dev_done_seq + ((q - 1) & Rm)) >= q;
+                        const uint32_t fm = __ballot_sync(0xffffffffu, fin);
+                        const uint32_t adv = (fm == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~fm) - 1);
+                        oldest += adv;
+                        if (adv < 32u) break;
+                    }
+                    if (oldest >= chain_next)
+                        quit = true;
+                    else
+                        last_activity = now;
+                }
             }
             if (quit) {
-                if (lane == 0) {
+                /* the host stops the engine only after everything has completed, and only a dispatcher that reads
+                 * the ring reads the host's stop word: the first to see it tells the others (quit word), lets the
+                 * service warps go and reports the exit */
+                if (lane == 0 && quit_word == 0u) {
+                    *reinterpret_cast<volatile uint32_t *>(g_quit) = 1u;
                     st_release_gpu(g_stop, 1ull);
                     __threadfence_system();
                     P.hctl[AESOFF_CTL_ALIVE] = 2;
@@ -520,86 +607,141 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             }
             continue;
         }
-        last_activity = globaltimer_ns();
 
-        /* ---- phase 2: lane k derives the geometry of request next_seq + k ---------------------- */
-        unsigned long long len = 0, rows = 0;
-        uint32_t nchunks = 0, crows = P.chunk_rows, fine = 0, nr = 0;
-        /* Latency modes.  A request of up to 64 KiB is always cut into 1/8-row units (32 blocks per
-         * warp; it is submission-bound anyway).  A larger one, up to fine_rows rows, is cut by the
-         * load it meets = rows not yet reserved by any CTA + the rows of this poll up to and including it:
-         *   - 1/8-row units while a quarter of the CTAs have nothing to do and the load makes at most two
-         *     waves of such units over the GPU's worker warps (a lone request: spread it over every
-         *     warp; 17 % more lookups per block, nobody is waiting for them);
-         *   - half rows while the load makes at most one and a half waves of half rows: half the time
-         *     per unit for 2.5 % more lookups;
-         *   - whole rows otherwise (saturation).                                                     */
-        const unsigned long long backlog = published > reserved ? published - reserved : 0ull;
-        const bool gpu_idle = idle * 4ull >= (unsigned long long)gridDim.x;
-        const unsigned long long warps = (unsigned long long)gridDim.x * AESOFF_WORKER_WARPS;
-        if (lane < n) {
+        /* ---- phase 2: what does not depend on the token: the rows of request pos + k ---------------- */
+        /* (32-bit row counts: the host refuses requests of 2^40 bytes and more) */
+        const bool mine = lane >= pos && lane < pos + n;
+        uint32_t rows = 0;
 #define PW(p) sw[AESOFF_PW_INDEX(p)]
-            /* only what the geometry needs; the rest goes from the staging area straight into dq */
-            len = ((unsigned long long)PW(AESOFF_PW_LEN + 1) << 32) | PW(AESOFF_PW_LEN);
-            nr = kw >> 24;
+        if (mine) {
+            const unsigned long long len = ((unsigned long long)PW(AESOFF_PW_LEN + 1) << 32) | PW(AESOFF_PW_LEN);
             const unsigned long long nblocks = (len >> 4) + ((len & 15ull) ? 1ull : 0ull);
             const uint32_t c0 = PW(AESOFF_PW_ICB + 3) >> 24;
-            rows = nblocks ? ((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0ull;
+            rows = nblocks ? (uint32_t)((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0u;
         }
         /* rows of this poll up to and including request k */
-        unsigned long long rows_incl = (lane < n) ? rows : 0ull;
+        uint32_t rows_incl = rows;
         if (n > 1) { /* a lone request (the latency case) skips the scan */
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const unsigned long long y = __shfl_up_sync(0xffffffffu, rows_incl, d);
-                if ((int)lane >= d) rows_incl += y;
+            for (int dd = 1; dd < 32; dd <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xffffffffu, rows_incl, dd);
+                if ((int)lane >= dd) rows_incl += y;
             }
         }
-        if (lane < n) {
-            const unsigned long long load = backlog * P.chunk_rows + rows_incl;
-            if (P.fine_rows && rows <= P.fine_rows) {
-                if (rows <= AESOFF_FINE_ALWAYS_ROWS || (gpu_idle && load * 8ull <= 2ull * warps)) {
-                    fine = AESOFF_FLAG_FINE;
-                    crows = crows > 1u ? crows / 2u : 1u;
-                } else if (load * 4ull <= 3ull * warps) {
-                    fine = AESOFF_FLAG_HALF;
-                }
+        const uint32_t rows_poll = __shfl_sync(0xffffffffu, rows_incl, n > 1 ? 31 : (int)pos);
+
+        /* ---- phase 3: the token -------------------------------------------------------------------- */
+        const unsigned long long my_next = b_seq + pos;
+        if (have_token) {
+            chain_pub = my_pub;
+        } else {
+            /* only the token is read again: the load figures of the poll are heuristics, and the line the
+             * ticket counter lives on belongs to the service warps' atomics */
+            while (chain_next != my_next) {
+                uint4 v = make_uint4(0, 0, 0, 0);
+                if (lane == 0) v = ld_volatile_v4(P.counters + AESOFF_CNT_CHAIN);
+                chain_pub = ((unsigned long long)__shfl_sync(0xffffffffu, v.y, 0) << 32) | __shfl_sync(0xffffffffu, v.x, 0);
+                chain_next = ((unsigned long long)__shfl_sync(0xffffffffu, v.w, 0) << 32) | __shfl_sync(0xffffffffu, v.z, 0);
             }
+        }
+        const unsigned long long published = chain_pub;
+#ifdef AESOFF_DISP_STATS
+        const unsigned long long dbg_t1 = globaltimer_ns();
+        dbg_wait += dbg_t1 - dbg_t0;
+        ++dbg_takes;
+#endif
+        /* Unit and chunk sizes by the load the request meets (all in 4 KiB rows; W = worker warps of the grid):
+         *   backlog   rows published and not yet reserved by any CTA (chunk_rows per ticket, roughly)
+         *   ahead     backlog + the rows of the requests before it in this poll
+         *   total     backlog + all rows of this poll: the queue as far as it is known
+         *   idle GPU  a quarter of the CTAs or more have no open slot
+         * Per chunk (the unit size travels in the ticket), r0 rows into its request:
+         *   1/8 rows   idle GPU, and the whole known queue is short (tune[FINE_TOTAL]) or the chunk is among its
+         *              first tune[FINE_FRONT] rows: spread it over every warp, nobody waits for the extra lookups
+         *   half rows  the known queue is at most tune[HALF_TOTAL] rows, or the request found at most tune[TAIL_AHEAD]
+         *              rows ahead of it and the chunk is among the last tune[TAIL_LEFT] rows of the queue (the end
+         *              of a long lone request must not be left to the few warps holding 2-row units)
+         *   rows       otherwise (saturation: 135.3 lookups per block instead of 139.75 / 160)
+         * Chunk = what one CTA takes at a time.  An idle CTA waits on ONE ticket that does not exist yet, so a request
+         * that finds (nearly) every CTA idle and at most tune[SPREAD_AHEAD] rows ahead is cut into one chunk per CTA,
+         * if that makes chunks of at most tune[SPREAD_MAX] rows: every CTA gets its share in the first round of
+         * ticket reads.  Otherwise a chunk is chunk_rows rows: small enough to balance, large enough that the
+         * service warps keep up.                                                                             */
+        uint32_t fine_max, half_min; /* the chunk that starts r0 rows into this lane's request: 1/8 rows if
+                                        (int)r0 <= fine_max, else half rows if (int)r0 >= half_min, else rows */
+        /* (the dispatcher is one warp running dependent instructions, a few clocks each: a hundred instructions
+         * on this path are 0.2 us on every request, so chunk sizes are powers of two and nothing here divides) */
+        uint32_t nchunks = 0, clog = P.chunk_log2; /* rows per chunk = 1 << clog */
+        {
+            const unsigned long long bl = (published > reserved ? published - reserved : 0ull) << P.chunk_log2;
+            const uint32_t backlog = bl > 0x3fffffffull ? 0x3fffffffu : (uint32_t)bl;
+            const uint32_t total_q = min(backlog + min(rows_poll, 0x3fffffffu), 0x3fffffffu);
+            const uint32_t ahead = min(backlog + (rows_incl - rows), 0x3fffffffu);
+            const bool may_cut = P.fine_rows != 0u && rows <= P.fine_rows;
+            const bool idle_gpu = idle * 4ull >= (unsigned long long)gridDim.x;
+            if (mine && may_cut && idle * 8ull >= 7ull * gridDim.x && ahead <= P.tune[AESOFF_TUNE_SPREAD_AHEAD] &&
+                rows <= gridDim.x * P.tune[AESOFF_TUNE_SPREAD_MAX]) { /* a lone request of moderate size */
+                /* longer requests keep chunk_rows: many tickets per CTA balance by themselves, and what a CTA may
+                 * hold is counted in chunk_rows-sized tickets (service_loop) */
+                clog = 0;
+                while ((gridDim.x << clog) < rows) ++clog;
+            }
+            int fm = -1, hm = 0x7fffffff;
+            if (may_cut) {
+                if (idle_gpu)
+                    fm = total_q <= P.tune[AESOFF_TUNE_FINE_TOTAL] ? 0x7fffffff
+                                                                   : (int)P.tune[AESOFF_TUNE_FINE_FRONT] - (int)ahead - (int)(1u << clog);
+                if (total_q <= P.tune[AESOFF_TUNE_HALF_TOTAL])
+                    hm = 0;
+                else if (ahead <= P.tune[AESOFF_TUNE_TAIL_AHEAD])
+                    hm = max(0, (int)(total_q - ahead) - (int)P.tune[AESOFF_TUNE_TAIL_LEFT]);
+            }
+            fine_max = (uint32_t)fm;
+            half_min = (uint32_t)hm;
+        }
+#define UNIT_MODE(fm_, hm_, r0_) ((int)(r0_) <= (int)(fm_) ? AESOFF_FLAG_FINE : (int)(r0_) >= (int)(hm_) ? AESOFF_FLAG_HALF : 0u)
+        if (mine) {
             /* a request must fit the ticket ring with room to spare */
-            const unsigned long long max_chunks = P.TM / 4;
-            while (((rows + crows - 1) / crows) > max_chunks) crows *= 2;
-            nchunks = (uint32_t)((rows + crows - 1) / crows);
+            while (((rows + (1u << clog) - 1u) >> clog) > P.TM / 4u) ++clog;
+            nchunks = (rows + (1u << clog) - 1u) >> clog;
         }
         /* exclusive prefix sum of nchunks -> first ticket of each request */
         uint32_t incl = nchunks;
         if (n > 1) {
 #pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const uint32_t y = __shfl_up_sync(0xffffffffu, incl, d);
-                if ((int)lane >= d) incl += y;
+            for (int dd = 1; dd < 32; dd <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xffffffffu, incl, dd);
+                if ((int)lane >= dd) incl += y;
             }
         }
         const unsigned long long first_ticket = published + incl - nchunks;
         /* ticket-ring capacity: every unfinished ticket must stay within TM of the newest.  `base`
          * is only refreshed (32 completion words per L2 round trip) when the cached one says no. */
         for (;;) {
-            const uint32_t fits = __ballot_sync(0xffffffffu, lane >= n || first_ticket + nchunks - base <= P.TM);
-            uint32_t nfit = (fits == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~fits) - 1);
-            if (nfit > n) nfit = n;
-            if (nfit == n) break;
+            const uint32_t fits = __ballot_sync(0xffffffffu, !mine || first_ticket + nchunks - base <= P.TM) >> pos;
+            uint32_t nfit = (~fits) ? (uint32_t)(__ffs(~fits) - 1) : 32u;
+            if (nfit >= n) break;
+            /* a ring slot is reused only after its previous request completed: whatever is a ring's length behind
+             * the request in hand needs no look (this bounds the scan after a long run without one) */
+            if (my_next > oldest + P.R) oldest = my_next - P.R;
             for (;;) {
                 const unsigned long long q = oldest + lane;
                 bool fin = false;
-                if (q < next_seq)
-                    fin = *reinterpret_cast<volatile uint64_t *>(P.dev_done_seq + ((q - 1) & Rm)) >= q;
+                if (q < my_next) fin = *reinterpret_cast<volatile uint64_t *>(P.dev_done_seq + ((q - 1) & Rm)) >= q;
                 const uint32_t fm = __ballot_sync(0xffffffffu, fin);
                 const uint32_t adv = (fm == 0xffffffffu) ? 32u : (uint32_t)(__ffs(~fm) - 1);
                 oldest += adv;
                 if (adv < 32u) break;
             }
-            unsigned long long nb = published;
-            if (lane == 0 && oldest < next_seq)
-                nb = *reinterpret_cast<volatile uint64_t *>(&P.dq[(oldest - 1) & Rm].w[24]); /* first_ticket: words 18, 19 */
+            /* first ticket of the oldest unfinished request: piece 6 of its device descriptor, which another
+             * dispatcher may not have written yet (then the tag is an older one, and the bound stays) */
+            unsigned long long nb = base;
+            if (oldest >= my_next) {
+                nb = published;
+            } else if (lane == 0) {
+                const uint4 v = ld_volatile_v4(&P.dq[(oldest - 1) & Rm].w[24]);
+                if (v.w == (uint32_t)oldest) nb = ((unsigned long long)v.y << 32) | v.x;
+            }
             nb = __shfl_sync(0xffffffffu, nb, 0);
             if (nb == base) {
                 if (nfit > 0) {
@@ -610,25 +752,48 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             }
             base = nb;
         }
-        if (lane >= n) nchunks = 0;
+        const bool take = lane >= pos && lane < pos + n;
+        if (!take) nchunks = 0;
+        const uint32_t total = __shfl_sync(0xffffffffu, incl, pos + n - 1);
+        /* pass the token on: everything below runs beside the other dispatchers */
+        const unsigned long long new_pub = published + total;
+        if (lane == 0) {
+            const unsigned long long nx = my_next + n;
+            asm volatile("st.volatile.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(g_chain), "r"((uint32_t)new_pub),
+                         "r"((uint32_t)(new_pub >> 32)), "r"((uint32_t)nx), "r"((uint32_t)(nx >> 32))
+                         : "memory");
+            /* what the service warps read.  Not a store: a dispatcher that got the token later may already
+             * have published a larger count.  No fence: the count only tells the service warps how many tickets
+             * they may reserve; a ticket is taken when its own 16-byte word shows up (tag).                  */
+            if (total) atomicMax(g_published, new_pub);
+        }
+        if (K > 1u && (wide != 0u) != queue_long) { /* as the holder: tell the others whether reading ahead pays */
+            queue_long = wide != 0u;
+            if (lane == 0) *(reinterpret_cast<volatile uint32_t *>(g_quit) + 1) = wide;
+        }
+        have_token = pos + n < 32u || K == 1u; /* still mine: nobody else can move it */
+        my_pub = new_pub;
+        token_at = my_next + n;
         if (n != n_seen) repoll = true; /* the ticket ring took fewer requests than the poll in flight assumes */
+
+        /* ---- phase 4: keys, descriptors, tickets ----------------------------------------------- */
+        const uint32_t fine = UNIT_MODE(fine_max, half_min, 0u); /* of the request's first chunk (statistics, descriptor) */
         {   /* statistics for aes_engine_info */
-            const uint32_t me = __ballot_sync(0xffffffffu, lane < n && (fine & AESOFF_FLAG_FINE));
-            const uint32_t mh = __ballot_sync(0xffffffffu, lane < n && (fine & AESOFF_FLAG_HALF));
+            const uint32_t me = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_FINE));
+            const uint32_t mh = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_HALF));
             n_eighths += __popc(me);
             n_halves += __popc(mh);
             n_rows += n - __popc(me) - __popc(mh);
             stats_dirty = true; /* written to the host when the ring is next found empty */
         }
-
-        /* ---- phase 3: keys, descriptors, tickets ----------------------------------------------- */
         uint32_t keyloc = kw & 0xffffu;
         if (!(kw & AESOFF_KW_RAW) && keyloc >= AESOFF_KEY_IDS) keyloc = AESOFF_KEY_IDS + slot; /* never sent by the host */
-        if (lane < n && (kw & AESOFF_KW_RAW)) {
+        if (take && (kw & AESOFF_KW_RAW)) {
             if (!(kw & AESOFF_KW_INSTALL) || keyloc >= AESOFF_KEY_IDS) keyloc = AESOFF_KEY_IDS + slot;
             uint32_t key[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) key[i] = PW(AESOFF_PW_RAWKEY + i);
+            const uint32_t nr = kw >> 24;
             if (nr == 10)
                 key_expand<4>(ybase, key, P.ktab[keyloc].rk); /* step a1 on the device */
             else if (nr == 12)
@@ -636,60 +801,77 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             else
                 key_expand<8>(ybase, key, P.ktab[keyloc].rk);
         }
-        if (lane < n) {
+        if (take) {
             /* the 24 descriptor words as 8 pieces of {3 words, tag}: see aesoff_dq_entry_t */
             uint4 *d4 = reinterpret_cast<uint4 *>(P.dq + slot);
             const uint32_t tg = (uint32_t)s;
             d4[0] = make_uint4(PW(AESOFF_PW_ICB + 0), PW(AESOFF_PW_ICB + 1), PW(AESOFF_PW_ICB + 2), tg);
             d4[1] = make_uint4(PW(AESOFF_PW_ICB + 3), PW(AESOFF_PW_SRC), PW(AESOFF_PW_SRC + 1), tg);
-            d4[2] = make_uint4(PW(AESOFF_PW_DST), PW(AESOFF_PW_DST + 1), (uint32_t)len, tg);
-            d4[3] = make_uint4((uint32_t)(len >> 32), nr, fine, tg);
-            d4[4] = make_uint4(nchunks, crows, (uint32_t)s, tg);
-            d4[5] = make_uint4((uint32_t)(s >> 32), (uint32_t)rows, (uint32_t)(rows >> 32), tg);
+            d4[2] = make_uint4(PW(AESOFF_PW_DST), PW(AESOFF_PW_DST + 1), PW(AESOFF_PW_LEN), tg);
+            d4[3] = make_uint4(PW(AESOFF_PW_LEN + 1), kw >> 24, fine, tg);
+            d4[4] = make_uint4(nchunks, 1u << clog, (uint32_t)s, tg);
+            d4[5] = make_uint4((uint32_t)(s >> 32), rows, 0u, tg);
             d4[6] = make_uint4((uint32_t)first_ticket, (uint32_t)(first_ticket >> 32), keyloc, tg);
             d4[7] = make_uint4(0u, 0u, 0u, tg);
         }
 #undef PW
         /* expanded keys (if any request of this poll brought a raw one) before the tickets that point at
          * them; descriptors need no fence, their pieces validate themselves */
-        if (__any_sync(0xffffffffu, lane < n && (kw & AESOFF_KW_RAW))) __threadfence();
+        if (__any_sync(0xffffffffu, take && (kw & AESOFF_KW_RAW))) __threadfence();
         __syncwarp();
         /* a request of up to eight chunks (the fine-grained regime: every request of the poll) gets its
          * tickets from its own lane; the warp then shares out the long ones, 32 tickets per step */
-        if (lane < n) {
-            const uint32_t md = fine << AESOFF_TICKET_MODE_SHIFT;
+        if (take) {
             for (uint32_t ch = 0; ch < nchunks && ch < 8u; ++ch) {
                 const unsigned long long tno = first_ticket + ch;
+                const uint32_t md = UNIT_MODE(fine_max, half_min, ch << clog) << AESOFF_TICKET_MODE_SHIFT;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
                     make_uint4((uint32_t)s, ch | md, keyloc, (uint32_t)tno + 1u);
             }
         }
-        for (uint32_t big = __ballot_sync(0xffffffffu, lane < n && nchunks > 8u); big; big &= big - 1u) {
+        for (uint32_t big = __ballot_sync(0xffffffffu, take && nchunks > 8u); big; big &= big - 1u) {
             const uint32_t k = __ffs(big) - 1;
             const uint32_t nc = __shfl_sync(0xffffffffu, nchunks, k);
             const unsigned long long ft = __shfl_sync(0xffffffffu, first_ticket, k);
             const uint32_t kl = __shfl_sync(0xffffffffu, keyloc, k);
-            const uint32_t md = __shfl_sync(0xffffffffu, fine, k) << AESOFF_TICKET_MODE_SHIFT;
-            const uint32_t sq = (uint32_t)(next_seq + k);
+            const uint32_t cl = __shfl_sync(0xffffffffu, clog, k);
+            const uint32_t fm = __shfl_sync(0xffffffffu, fine_max, k), hm = __shfl_sync(0xffffffffu, half_min, k);
+            const uint32_t sq = (uint32_t)(b_seq + k);
             for (uint32_t ch = 8u + lane; ch < nc; ch += 32) {
                 const unsigned long long tno = ft + ch;
+                const uint32_t md = UNIT_MODE(fm, hm, ch << cl) << AESOFF_TICKET_MODE_SHIFT;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
                     make_uint4(sq, ch | md, kl, (uint32_t)tno + 1u);
             }
         }
-        const uint32_t total = __shfl_sync(0xffffffffu, incl, n - 1);
+#undef UNIT_MODE
         __syncwarp();
-        published += total;
-        /* No fence here: the published count only tells the service warps how many tickets they may
-         * reserve; a ticket is taken when its own 16-byte word shows up (tag), whichever arrives first. */
-        if (lane == 0 && total) *reinterpret_cast<volatile unsigned long long *>(g_published) = published;
         /* an empty request (len == 0) has no ticket: complete it here */
-        if (lane < n && nchunks == 0) {
+        if (take && nchunks == 0) {
             __threadfence_system();
             P.hmail[slot] = s;
             *reinterpret_cast<volatile uint64_t *>(P.dev_done_seq + slot) = s;
         }
-        next_seq += n;
+#ifdef AESOFF_DISP_STATS
+        dbg_reqs += n;
+        dbg_work += globaltimer_ns() - dbg_t1;
+#endif
+#ifndef AESOFF_EARLY_PREFETCH
+        /* the next poll, after the last ticket store: issuing the copies takes a quarter of a microsecond that a lone
+         * request would otherwise wait for; under load the poll still flies while the service warps pick the
+         * tickets up and while this warp does the look and the token of the next batch */
+        if (n == n_seen) {
+            if (pos + n == 32u)
+                ISSUE_POLL(b_seq + (unsigned long long)AESOFF_BATCH * K, 0u, true);
+            else
+                ISSUE_POLL(b_seq, pos + n, true);
+        }
+#endif
+        pos += n;
+        if (pos == 32u) {
+            pos = 0;
+            b_seq += (unsigned long long)AESOFF_BATCH * K;
+        }
     }
 }
 
@@ -709,8 +891,8 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
     CtaCtl *c = reinterpret_cast<CtaCtl *>(smem + (ctrl - sbase));
 
 #ifdef AESOFF_DEBUG
-#define DBG_MIN(i) do { if (tid == 0 || (tid & 31u) == 0) atomicMin(reinterpret_cast<unsigned long long *>(P.counters) + 20 + (i), globaltimer_ns()); } while (0)
-#define DBG_MAX(i) do { if (tid == 0 || (tid & 31u) == 0) atomicMax(reinterpret_cast<unsigned long long *>(P.counters) + 20 + (i), globaltimer_ns()); } while (0)
+#define DBG_MIN(i) do { if (tid == 0 || (tid & 31u) == 0) atomicMin(reinterpret_cast<unsigned long long *>(P.counters) + AESOFF_CNT_DEBUG + (i), globaltimer_ns()); } while (0)
+#define DBG_MAX(i) do { if (tid == 0 || (tid & 31u) == 0) atomicMax(reinterpret_cast<unsigned long long *>(P.counters) + AESOFF_CNT_DEBUG + (i), globaltimer_ns()); } while (0)
 #else
 #define DBG_MIN(i) ((void)0)
 #define DBG_MAX(i) ((void)0)
@@ -727,7 +909,7 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
         service_loop(P, c, lane);
     } else if (warp == AESOFF_WORKER_WARPS + 1) {
         asm volatile("bar.sync 1, %0;" ::"n"(AESOFF_CTA_THREADS) : "memory");
-        if (P.mode == AESOFF_MODE_PERSISTENT && blockIdx.x == 0) dispatcher_loop(P, c, tbase | (lane * 4u), lane);
+        if (P.mode == AESOFF_MODE_PERSISTENT && blockIdx.x < P.n_disp) dispatcher_loop(P, c, tbase | (lane * 4u), lane, blockIdx.x);
     } else {
         if (tid == 0 && blockIdx.x == 0 && P.hctl) P.hctl[AESOFF_CTL_SMEMBASE] = sbase;
         fill_tables(tbase, P.T0, tid, AESOFF_WORKER_WARPS * 32u); /* worker threads only */

@@ -49,6 +49,13 @@ static inline void store_piece(uint32_t *dst, uint32_t a, uint32_t b, uint32_t c
 namespace {
 
 thread_local int t_last_error = AES_OK;
+/* executor threads spread over the shards of per-thread counters */
+inline int thread_shard()
+{
+    static std::atomic<int> next{0};
+    thread_local int mine = next.fetch_add(1, std::memory_order_relaxed);
+    return mine & 15;
+}
 inline int fail(int code)
 {
     t_last_error = code;
@@ -62,11 +69,20 @@ inline uint64_t now_ns()
     return (uint64_t)ts.tv_sec * 1000000000ull + (uint64_t)ts.tv_nsec;
 }
 
+constexpr int SUBMIT_SHARDS = 16;
+struct alignas(64) SubmitShard {
+    std::atomic<int> n{0};
+};
+
 struct Engine {
-    std::atomic<int> running{0};
+    /* Cache-line hygiene for executor pools (32 threads): next_seq is claimed by every submit, so
+     * it sits on a line of its own; what every submit and poll only READS (geometry, pointers, running,
+     * done_upto) never shares a line with it; the in-flight count is sharded by thread.                   */
+    alignas(64) std::atomic<int> running{0};
     int device = -1;
     int sm_count = 0;
     int n_ctas = 0;
+    uint32_t n_disp = 1;
     uint32_t R = 0, Rm = 0, chunk_rows = 0, TM = 0;
     cudaStream_t stream = nullptr;
     aesoff_host_slot_t *hring = nullptr; /* pinned, mapped */
@@ -78,16 +94,17 @@ struct Engine {
     uint64_t *counters = nullptr, *dev_done_seq = nullptr;
     uint32_t *dq_done = nullptr, *dT0 = nullptr;
     uint64_t first_seq = 1;               /* first sequence number of the current run          */
-    std::atomic<uint64_t> next_seq{1};    /* next sequence number to hand out (never reset)    */
+    alignas(64) std::atomic<uint64_t> next_seq{1}; /* next sequence number to hand out (never reset) */
+    alignas(64) SubmitShard submitters[SUBMIT_SHARDS];
     /* ktab indices for installed contexts.  An index freed while next_seq == s is handed out again
      * only once next_seq >= s + R: by then every request that could name it has completed (a ring
      * slot is reused only after its previous request completed).                                  */
-    std::mutex id_mu;
+    alignas(64) std::mutex id_mu;
     std::deque<std::pair<uint32_t, uint64_t>> id_free; /* (index, next_seq when freed), FIFO   */
     std::atomic<uint64_t> k_epoch{1};     /* bumped whenever ktab is (re)allocated             */
-    /* aes_ctr_submit calls between their `running` check and their last slot store: aes_engine_stop waits
-     * for this to reach 0 before it reads next_seq, so no sequence number is published behind its back */
-    std::atomic<int> submitters{0};
+    /* submitters[]: aes_ctr_submit calls between their `running` check and their last slot store, counted per
+     * thread shard: aes_engine_stop waits for all of them to reach 0 before it reads next_seq, so no sequence
+     * number is published behind its back */
     /* every sequence number below this belongs to a run that has been stopped: complete, unless listed
      * in `lost` (requests an unclean stop -- dead kernel -- never saw complete)                        */
     std::atomic<uint64_t> done_upto{1};
@@ -177,6 +194,7 @@ int check_buffers(const void *src, void *dst, size_t len)
 {
     if (len == 0) return AES_OK;
     if (!src || !dst) return AES_E_INVAL;
+    if ((uint64_t)len >= (1ull << 36)) return AES_E_INVAL; /* 64 GiB: the dispatcher counts 4 KiB rows in 32 bits */
     const uintptr_t s = (uintptr_t)src, d = (uintptr_t)dst;
     if ((s | d) & 15u) return AES_E_ALIGN;
     if (s != d && s < d + len && d < s + len) return AES_E_OVERLAP;
@@ -238,6 +256,7 @@ extern "C" aes_ctx_t *aes_ctx_create(const uint8_t *key, int keybits)
     c->state = AESOFF_CTX_FRESH;
     c->id = AESOFF_KEY_NONE;
     c->epoch = 0;
+    c->install_seq = 0;
     return c;
 }
 
@@ -301,13 +320,15 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     aes_engine_opts_t o;
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
-    for (int i = 0; i < 3; ++i)
+    for (int i = 0; i < 2; ++i)
         if (o.reserved[i]) return fail(AES_E_INVAL);
+    if (o.n_dispatchers == 0) o.n_dispatchers = AESOFF_DEF_DISPATCHERS;
+    if (o.n_dispatchers > AESOFF_MAX_DISPATCHERS) return fail(AES_E_INVAL);
     if (o.ring_slots == 0) o.ring_slots = 2048;
     if (o.chunk_rows == 0) o.chunk_rows = 4;
     if (!is_pow2(o.ring_slots) || o.ring_slots < 64 || o.ring_slots > 4096) return fail(AES_E_INVAL);
-    if (o.chunk_rows > 64) return fail(AES_E_INVAL);
-    if (o.fine_rows == 0) o.fine_rows = 2048;
+    if (o.chunk_rows > 64 || !is_pow2(o.chunk_rows)) return fail(AES_E_INVAL);
+    if (o.fine_rows == 0) o.fine_rows = 0xfffffffeu;
     if (o.fine_rows == AES_FINE_ROWS_OFF) o.fine_rows = 0;
 
     int ndev = 0;
@@ -326,6 +347,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     e.device = device;
     e.sm_count = sms;
     e.n_ctas = o.n_ctas ? (int)o.n_ctas : sms;
+    e.n_disp = o.n_dispatchers < (uint32_t)e.n_ctas ? o.n_dispatchers : (uint32_t)e.n_ctas;
     e.R = o.ring_slots;
     e.Rm = e.R - 1;
     e.chunk_rows = o.chunk_rows;
@@ -360,6 +382,9 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     /* sequence numbers never restart, so stale slot/mailbox values (< first_seq) can never match */
     memset(e.hctl, 0, AESOFF_CTL_WORDS * 4);
     ok = ok && cudaMemsetAsync(e.counters, 0, AESOFF_CNT_WORDS * 8, e.stream) == cudaSuccess;
+    /* the dispatchers' token: no ticket published yet, the first request to dispatch is first_seq */
+    const uint64_t chain0[2] = {0ull, e.first_seq};
+    ok = ok && cudaMemcpyAsync(e.counters + AESOFF_CNT_CHAIN, chain0, 16, cudaMemcpyHostToDevice, e.stream) == cudaSuccess;
     ok = ok && cudaMemsetAsync(e.dq_done, 0, (size_t)e.R * 4, e.stream) == cudaSuccess;
     /* ticket numbers restart from 0 with every launch: no stale ticket may carry a matching tag */
     ok = ok && cudaMemsetAsync(e.tmap, 0, (size_t)e.TM * sizeof(aesoff_ticket_t), e.stream) == cudaSuccess;
@@ -383,10 +408,31 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     p.R = e.R;
     p.TM = e.TM;
     p.chunk_rows = e.chunk_rows;
+    for (p.chunk_log2 = 0; (1u << p.chunk_log2) < e.chunk_rows; ++p.chunk_log2) {}
     p.mode = AESOFF_MODE_PERSISTENT;
     p.idle_exit_ms = o.idle_exit_ms;
     p.fine_rows = o.fine_rows;
     p.first_seq = e.first_seq;
+    p.n_disp = e.n_disp;
+    {   /* unit-size policy thresholds in rows (aesoff_shared.h AESOFF_TUNE_*); W = worker warps of the grid.
+         * AESOFF_TUNE="a,b,c,d,e,f,g" overrides them (tuning experiments only). */
+        const uint32_t W = (uint32_t)e.n_ctas * AESOFF_WORKER_WARPS;
+        p.tune[AESOFF_TUNE_FINE_TOTAL] = W / 4;
+        p.tune[AESOFF_TUNE_FINE_FRONT] = 0;
+        p.tune[AESOFF_TUNE_HALF_TOTAL] = 3 * W / 4;
+        p.tune[AESOFF_TUNE_TAIL_AHEAD] = W;
+        p.tune[AESOFF_TUNE_TAIL_LEFT] = 2 * W;
+        p.tune[AESOFF_TUNE_SPREAD_AHEAD] = W / 2;
+        p.tune[AESOFF_TUNE_SPREAD_MAX] = 16;
+        if (const char *t = getenv("AESOFF_TUNE")) {
+            for (int i = 0; i < 7 && t && *t; ++i) {
+                char *end = nullptr;
+                const unsigned long v = strtoul(t, &end, 10);
+                if (end != t) p.tune[i] = (uint32_t)v;
+                t = (*end == ',') ? end + 1 : nullptr;
+            }
+        }
+    }
     if (aesoff_launch_engine(&p, e.n_ctas, e.stream) != 0) {
         free_engine_memory(e);
         return fail(AES_E_CUDA);
@@ -420,7 +466,8 @@ extern "C" int aes_engine_stop(void)
     if (!e.running.load()) return fail(AES_E_STOPPED);
     /* no new submissions from here on; the ones that passed their `running` check finish publishing */
     e.running.store(2, std::memory_order_seq_cst);
-    while (e.submitters.load(std::memory_order_seq_cst) != 0) CPU_RELAX();
+    for (int i = 0; i < SUBMIT_SHARDS; ++i)
+        while (e.submitters[i].n.load(std::memory_order_seq_cst) != 0) CPU_RELAX();
     int rc = AES_OK;
     /* drain: every accepted request completes (unless the kernel died) */
     const uint64_t last = e.next_seq.load();
@@ -445,6 +492,8 @@ extern "C" int aes_engine_stop(void)
             if (__atomic_load_n(&e.hmail[(s - 1) & e.Rm], __ATOMIC_ACQUIRE) < s) e.lost.push_back(s);
         if (e.lost.size() > 65536) e.lost.erase(e.lost.begin(), e.lost.end() - 65536);
         e.any_lost.store(e.lost.empty() ? 0 : 1, std::memory_order_release);
+        /* a lost request may be one that was to file a key in ktab: every installed context installs again */
+        reset_key_ids(e);
     }
     e.done_upto.store(last, std::memory_order_release);
     /* ring, mailbox and queues are kept for the next start (aes_poll may still be reading the mailbox);
@@ -478,12 +527,28 @@ extern "C" int aes_engine_info(aes_engine_info_t *out)
     }
     out->completed = out->submitted - pending;
     out->kernel_launches = g_kernel_launches.load();
+    out->n_dispatchers = e.n_disp;
     if (e.hctl) {
-        out->cut_eighths = __atomic_load_n(&e.hctl[AESOFF_CTL_CUT_EIGHTHS], __ATOMIC_RELAXED);
-        out->cut_halves = __atomic_load_n(&e.hctl[AESOFF_CTL_CUT_HALVES], __ATOMIC_RELAXED);
-        out->cut_rows = __atomic_load_n(&e.hctl[AESOFF_CTL_CUT_ROWS], __ATOMIC_RELAXED);
+        for (uint32_t d = 0; d < AESOFF_MAX_DISPATCHERS; ++d) { /* one set per dispatcher warp */
+            const uint32_t *st = e.hctl + AESOFF_CTL_STATS + AESOFF_CTL_STAT_WORDS * d;
+            out->cut_eighths += __atomic_load_n(&st[AESOFF_CTL_CUT_EIGHTHS], __ATOMIC_RELAXED);
+            out->cut_halves += __atomic_load_n(&st[AESOFF_CTL_CUT_HALVES], __ATOMIC_RELAXED);
+            out->cut_rows += __atomic_load_n(&st[AESOFF_CTL_CUT_ROWS], __ATOMIC_RELAXED);
+        }
     }
     return AES_OK;
+}
+
+/* AESOFF_DISP_STATS builds: per-dispatcher counters (polls that took requests, requests, token wait and work
+ * in units of 64 ns, empty polls), 5 words per dispatcher; zeros otherwise.  Tuning aid, not in aesoff.h.   */
+extern "C" __attribute__((visibility("default"))) int aesoff_debug_dispatch_stats(uint32_t out[5 * AESOFF_MAX_DISPATCHERS])
+{
+    Engine &e = g_eng;
+    if (!e.hctl) return -1;
+    for (uint32_t d = 0; d < AESOFF_MAX_DISPATCHERS; ++d)
+        for (int i = 0; i < 5; ++i)
+            out[5 * d + i] = __atomic_load_n(&e.hctl[AESOFF_CTL_STATS + AESOFF_CTL_STAT_WORDS * d + AESOFF_CTL_DBG_TAKES + i], __ATOMIC_RELAXED);
+    return 0;
 }
 
 /* ============================================================================================ */
@@ -508,29 +573,39 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
         std::atomic<int> &n;
         explicit InFlight(std::atomic<int> &c) : n(c) { n.fetch_add(1, std::memory_order_seq_cst); }
         ~InFlight() { n.fetch_sub(1, std::memory_order_seq_cst); }
-    } in_flight(e.submitters);
+    } in_flight(e.submitters[thread_shard()].n);
     if (e.running.load(std::memory_order_seq_cst) != 1 || engine_dead(e)) {
         fail(AES_E_STOPPED);
         return 0;
     }
-    /* how the key travels (aesoff_internal.h): raw the first two times, by ktab index afterwards.
-     * Decided BEFORE the sequence number is claimed: a submit that sees INSTALLED then gets a number
-     * above the installing one, and the dispatcher takes requests in sequence order.              */
+    /* how the key travels (aesoff_internal.h): raw until the request that files the expanded key in ktab
+     * has completed, by ktab index afterwards.  Completion is what orders the two: the dispatcher warps take
+     * batches of requests side by side, so a lower sequence number alone does not mean "expanded first". */
     uint32_t kw = ((uint32_t)ctx->nr << 24) | AESOFF_KEY_NONE | AESOFF_KW_RAW;
     bool installing = false;
     uint32_t st = __atomic_load_n(&ctx->state, __ATOMIC_ACQUIRE);
-    if (st == AESOFF_CTX_INSTALLED && ctx->epoch == e.k_epoch.load(std::memory_order_acquire)) {
+    const uint64_t epoch_now = e.k_epoch.load(std::memory_order_acquire);
+    const bool epoch_ok = __atomic_load_n(&ctx->epoch, __ATOMIC_ACQUIRE) == epoch_now;
+    if (st == AESOFF_CTX_INSTALLING && epoch_ok) {
+        const uint64_t is = __atomic_load_n(&ctx->install_seq, __ATOMIC_ACQUIRE);
+        if (is != 0 && __atomic_load_n(&e.hmail[(is - 1) & e.Rm], __ATOMIC_ACQUIRE) >= is) {
+            __atomic_store_n(&ctx->state, AESOFF_CTX_INSTALLED, __ATOMIC_RELEASE);
+            st = AESOFF_CTX_INSTALLED;
+        }
+    }
+    if (st == AESOFF_CTX_INSTALLED && epoch_ok) {
         kw = ((uint32_t)ctx->nr << 24) | ctx->id;
     } else if (st == AESOFF_CTX_FRESH) {
         __atomic_compare_exchange_n(&ctx->state, &st, AESOFF_CTX_SEEN, false, __ATOMIC_ACQ_REL, __ATOMIC_ACQUIRE);
-    } else if (st == AESOFF_CTX_SEEN || st == AESOFF_CTX_INSTALLED) {
+    } else if (st == AESOFF_CTX_SEEN || (st == AESOFF_CTX_INSTALLED && !epoch_ok)) {
         /* INSTALLED under an older ktab generation (the engine was rebuilt): install again */
         const uint32_t id = alloc_key_id(e);
         if (id != AESOFF_KEY_NONE) {
             if (__atomic_compare_exchange_n(&ctx->state, &st, AESOFF_CTX_INSTALLING, false, __ATOMIC_ACQ_REL,
                                             __ATOMIC_ACQUIRE)) {
+                __atomic_store_n(&ctx->install_seq, 0ull, __ATOMIC_RELEASE);
                 ctx->id = id;
-                ctx->epoch = e.k_epoch.load(std::memory_order_acquire);
+                __atomic_store_n(&ctx->epoch, epoch_now, __ATOMIC_RELEASE);
                 kw |= AESOFF_KW_INSTALL;
                 kw = (kw & ~0xffffu) | id;
                 installing = true;
@@ -539,7 +614,7 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
                 e.id_free.emplace_front(id, 0ull);
             }
         }
-    }
+    } /* else: INSTALLING and not complete yet (or another thread is in the middle of it): raw, nothing stored */
     /* claim the next sequence number, but only if its slot has been vacated */
     uint64_t s = e.next_seq.load(std::memory_order_acquire);
     for (;;) {
@@ -551,6 +626,7 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
                     e.id_free.emplace_front(ctx->id, 0ull);
                 }
                 ctx->id = AESOFF_KEY_NONE;
+                __atomic_store_n(&ctx->epoch, 0ull, __ATOMIC_RELEASE);
                 __atomic_store_n(&ctx->state, AESOFF_CTX_SEEN, __ATOMIC_RELEASE);
             }
             fail(AES_E_AGAIN);
@@ -581,15 +657,22 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
     store_piece(w + 4, icb[3], (uint32_t)a_src, (uint32_t)(a_src >> 32), tag);
     store_piece(w + 8, (uint32_t)a_dst, (uint32_t)(a_dst >> 32), (uint32_t)a_len, tag);
     store_piece(w + 12, (uint32_t)(a_len >> 32), kw, 0u, tag);
-    /* a later submit may name ktab[id] only after this one, which installs it, has a lower seq */
-    if (installing) __atomic_store_n(&ctx->state, AESOFF_CTX_INSTALLED, __ATOMIC_RELEASE);
+    /* later submits name ktab[id] once this request, which fills it, has completed */
+    if (installing) __atomic_store_n(&ctx->install_seq, s, __ATOMIC_RELEASE);
     return (aes_handle_t)s;
 }
 
 extern "C" int aes_poll(aes_handle_t h)
 {
     Engine &e = g_eng;
-    if (h == 0 || h >= e.next_seq.load(std::memory_order_acquire)) return fail(AES_E_INVAL);
+    /* A valid handle is below next_seq.  That word is claimed by every submit of every thread, so a poll does
+     * not read it: it compares with this thread's last copy and refreshes the copy only for a handle above it. */
+    thread_local uint64_t seen_next = 0;
+    if (h == 0) return fail(AES_E_INVAL);
+    if (h >= seen_next) {
+        seen_next = e.next_seq.load(std::memory_order_acquire);
+        if (h >= seen_next) return fail(AES_E_INVAL);
+    }
     if (h < e.done_upto.load(std::memory_order_acquire)) {
         /* a run that has been stopped: a clean stop drained everything, an unclean one lists what it lost */
         if (e.any_lost.load(std::memory_order_acquire)) {
@@ -887,6 +970,37 @@ extern "C" __attribute__((visibility("default"))) int aesoff_debug_stamps(uint64
 /* ============================================================================================ */
 /* closed-loop executor (PAPER.md:127-135 worker loop; "50 concurrent clients")      */
 /* ============================================================================================ */
+namespace {
+/* Per-request time stamps of the executors: two clock_gettime calls per request are half of what a 4 KiB
+ * request costs the submitting thread, so on x86 the loops read the time stamp counter and convert with a
+ * factor measured once against CLOCK_MONOTONIC_RAW.                                                     */
+struct TickClock {
+    double ns_per_tick = 1.0;
+    TickClock()
+    {
+#if defined(__x86_64__)
+        const uint64_t t0 = now_ns(), c0 = __rdtsc();
+        while (now_ns() - t0 < 2000000ull) CPU_RELAX();
+        const uint64_t t1 = now_ns(), c1 = __rdtsc();
+        ns_per_tick = (double)(t1 - t0) / (double)(c1 - c0);
+#endif
+    }
+};
+inline uint64_t ticks()
+{
+#if defined(__x86_64__)
+    return __rdtsc();
+#else
+    return now_ns();
+#endif
+}
+inline double tick_ns()
+{
+    static const TickClock clk;
+    return clk.ns_per_tick;
+}
+} /* namespace */
+
 extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res, double *lat_ns)
 {
     if (!spec || !res || !spec->nonces || !spec->srcs || !spec->dsts || !spec->lens) return fail(AES_E_INVAL);
@@ -898,13 +1012,21 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
     const uint64_t repeat = spec->repeat ? spec->repeat : 1;
     const uint64_t total = (uint64_t)spec->n * repeat;
     const uint32_t window = spec->window > e.R ? e.R : spec->window;
+    const double nspt = tick_ns();
 
+    /* In flight, in submission order.  Completions come roughly in that order, so a sweep polls from the oldest
+     * and gives up after 32 requests that are still pending (every eighth sweep looks at all of them): a window
+     * of 256 costs a few polls per completion, not 256.  A request that completed out of order stays in the
+     * queue as a tombstone until the ones before it are gone.                                              */
     struct Fly {
         aes_handle_t h;
         uint64_t t_submit;
         uint64_t index;
     };
-    std::vector<Fly> fly(window);
+    size_t cap = 64;
+    while (cap < 4 * (size_t)window) cap <<= 1;
+    std::vector<Fly> q(cap);
+    uint64_t head = 0, tail = 0, sweep = 0;
     uint32_t n_fly = 0;
     uint64_t next = 0, done = 0, bytes = 0;
     memset(res, 0, sizeof(*res));
@@ -912,14 +1034,14 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
     const uint64_t t_begin = now_ns();
     while (done < total) {
         /* submit until the window is full */
-        while (n_fly < window && next < total) {
+        while (n_fly < window && next < total && tail - head < cap) {
             const size_t i = (size_t)(next % spec->n);
             aes_ctx_t *ctx = spec->ctx;
             if (spec->keys) {
                 ctx = aes_ctx_create(spec->keys + 32 * i, spec->keybits[i]);
                 if (!ctx) return t_last_error;
             }
-            const uint64_t ts = now_ns();
+            const uint64_t ts = lat_ns ? ticks() : 0;
             const aes_handle_t h = aes_ctr_submit(ctx, spec->nonces + 16 * i, spec->srcs[i], spec->dsts[i], spec->lens[i]);
             if (spec->keys) aes_ctx_destroy(ctx);
             if (h == 0) {
@@ -929,25 +1051,30 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
                 }
                 return t_last_error;
             }
-            fly[n_fly++] = Fly{h, ts, next};
-            if (n_fly > res->max_in_flight) res->max_in_flight = n_fly;
+            q[tail++ & (cap - 1)] = Fly{h, ts, next};
+            if (++n_fly > res->max_in_flight) res->max_in_flight = n_fly;
             ++next;
         }
-        /* poll everything in flight; compact the array as completions are seen */
-        uint32_t k = 0;
-        while (k < n_fly) {
-            const int r = aes_poll(fly[k].h);
+        /* poll from the oldest */
+        const bool all = (++sweep & 7u) == 0;
+        uint32_t pending = 0;
+        for (uint64_t k = head; k < tail; ++k) {
+            Fly &f = q[k & (cap - 1)];
+            if (f.h == 0) continue; /* tombstone */
+            const int r = aes_poll(f.h);
             if (r == 1) {
-                if (lat_ns) lat_ns[fly[k].index] = (double)(now_ns() - fly[k].t_submit);
-                bytes += spec->lens[fly[k].index % spec->n];
+                if (lat_ns) lat_ns[f.index] = (double)(ticks() - f.t_submit) * nspt;
+                bytes += spec->lens[f.index % spec->n];
                 ++done;
-                fly[k] = fly[--n_fly];
+                --n_fly;
+                f.h = 0;
             } else if (r < 0) {
                 return r;
-            } else {
-                ++k;
+            } else if (++pending >= 32u && !all) {
+                break;
             }
         }
+        while (head < tail && q[head & (cap - 1)].h == 0) ++head;
     }
     res->elapsed_ns = now_ns() - t_begin;
     res->bytes = bytes;

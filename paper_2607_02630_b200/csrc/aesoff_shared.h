@@ -49,17 +49,33 @@
 #define AESOFF_CTL_STOP        0      /* host -> device: 1 = exit after the ring is drained */
 #define AESOFF_CTL_ALIVE       1      /* device -> host: 1 once the kernel polls, 2 after it exits */
 #define AESOFF_CTL_SMEMBASE    2      /* device -> host: shared-window offset of dynamic smem (debug) */
-#define AESOFF_CTL_CUT_EIGHTHS 4      /* device -> host: requests cut into 1/8-row units so far (statistics) */
-#define AESOFF_CTL_CUT_HALVES  5      /*                 ... into half rows                                  */
-#define AESOFF_CTL_CUT_ROWS    6      /*                 ... into whole rows                                 */
-#define AESOFF_CTL_WORDS       16
+#define AESOFF_CTL_STATS       16     /* device -> host, 8 words per dispatcher warp d at 16 + 8 d (statistics): */
+#define AESOFF_CTL_CUT_EIGHTHS 0      /*   requests whose first chunk was cut into 1/8-row units so far          */
+#define AESOFF_CTL_CUT_HALVES  1      /*   ... into half rows                                                    */
+#define AESOFF_CTL_CUT_ROWS    2      /*   ... into whole rows                                                   */
+#define AESOFF_MAX_DISPATCHERS 8u     /* dispatcher warps (warp 17 of CTAs 0 .. n-1); default AESOFF_DEF_DISPATCHERS */
+#define AESOFF_DEF_DISPATCHERS 2u
+#define AESOFF_BATCH           32u    /* consecutive sequence numbers one dispatcher takes: batch b belongs to dispatcher b % n */
+#define AESOFF_CTL_DBG_TAKES   3      /*   (AESOFF_DISP_STATS builds) polls that took requests, ...              */
+#define AESOFF_CTL_DBG_REQS    4      /*   ... requests taken, ...                                               */
+#define AESOFF_CTL_DBG_WAIT    5      /*   ... time spent waiting for the token, in units of 64 ns, ...          */
+#define AESOFF_CTL_DBG_WORK    6      /*   ... time from the token to the last ticket store, in units of 64 ns   */
+#define AESOFF_CTL_DBG_EMPTY   7      /*   ... polls that found nothing                                          */
+#define AESOFF_CTL_STAT_WORDS  8
+#define AESOFF_CTL_WORDS       128
 
 /* device counters (index in uint64 units) */
 #define AESOFF_CNT_TICKET      0      /* next ticket to hand out (atomicAdd by the service warps)      */
 #define AESOFF_CNT_PUBLISHED   1      /* tickets the dispatcher has published; same 16 B as TICKET      */
 #define AESOFF_CNT_IDLE        8      /* CTAs of the persistent engine that have no open slot           */
+#define AESOFF_CNT_QUIT        9      /* low half: dispatcher 0 -> the others: leave (idle timer); high half: the dispatcher
+                                         that holds the token found a long queue (the others prefetch their batches);
+                                         same 16 B as IDLE */
 #define AESOFF_CNT_STOP        16
-#define AESOFF_CNT_WORDS       32
+#define AESOFF_CNT_DEBUG       20     /* 8 words of time stamps in AESOFF_DEBUG builds                   */
+#define AESOFF_CNT_CHAIN       32     /* {tickets published, next sequence number to dispatch}: the token the
+                                         dispatcher warps pass along, one 16-byte word on a line of its own */
+#define AESOFF_CNT_WORDS       64
 
 /* ---- host ring slot: 8 pieces of {payload[3], tag}; tag = (uint32_t)seq -------------------- */
 /* payload word p (0..23) of a slot is w[(p / 3) * 4 + p % 3]                                    */
@@ -123,6 +139,15 @@ typedef struct __attribute__((aligned(16))) aesoff_ticket {
     uint32_t tag;          /* (uint32_t)ticket number + 1; the ring is zeroed at engine start          */
 } aesoff_ticket_t;         /* 16 bytes, written and read as one 128-bit access                         */
 
+/* unit-size policy of the persistent dispatcher; W = worker warps of the grid */
+#define AESOFF_TUNE_FINE_TOTAL   0    /* idle GPU, whole known queue at most this many rows: 1/8-row units (W / 4) */
+#define AESOFF_TUNE_FINE_FRONT   1    /* idle GPU: the first this many rows of the queue in 1/8 rows     (0: off) */
+#define AESOFF_TUNE_HALF_TOTAL   2    /* known queue at most this many rows: half rows                   (3 W / 4) */
+#define AESOFF_TUNE_TAIL_AHEAD   3    /* a request that found at most this many rows ahead of it ...     (W)     */
+#define AESOFF_TUNE_TAIL_LEFT    4    /* ... has its last this many rows cut into half rows              (2 W)   */
+#define AESOFF_TUNE_SPREAD_AHEAD 5    /* idle GPU and at most this many rows ahead: one chunk per CTA ... (W / 2) */
+#define AESOFF_TUNE_SPREAD_MAX   6    /* ... of at most this many rows                                   (16)    */
+
 typedef struct aesoff_params {
     aesoff_host_slot_t *hring;      /* host-mapped (persistent mode)                     */
     volatile uint64_t  *hmail;      /* host-mapped mailbox, may be NULL in drain mode    */
@@ -138,10 +163,13 @@ typedef struct aesoff_params {
     uint32_t            R;          /* ring slots, power of two                          */
     uint32_t            TM;         /* ticket ring entries, power of two                 */
     uint32_t            chunk_rows;
+    uint32_t            chunk_log2; /* chunk_rows == 1 << chunk_log2 */
     uint32_t            mode;
     uint32_t            idle_exit_ms;
-    uint32_t            fine_rows;  /* requests of at most this many rows may be cut into 1/8-row units; 0 = never */
+    uint32_t            fine_rows;  /* requests of at most this many rows may be cut into units smaller than a row; 0 = never */
     uint64_t            first_seq;  /* sequence number of the first request of this launch */
+    uint32_t            n_disp;     /* dispatcher warps (persistent mode), 1 .. AESOFF_MAX_DISPATCHERS      */
+    uint32_t            tune[7];    /* unit-size policy thresholds in rows, AESOFF_TUNE_* (dispatcher_loop) */
 } aesoff_params_t;
 
 #endif

@@ -120,6 +120,17 @@ def test_fails_loudly_without_engine_or_gpu(P):
     P.aes_ctx_destroy(ctx)
 
 
+def test_engine_options_are_validated_before_any_cuda_call():
+    """Bad option values are AES_E_INVAL whether or not there is a GPU: chunk_rows must be a power of two up to 64,
+    at most 8 dispatcher warps, the ring a power of two in [64, 4096]."""
+    import paper_2607_02630_b200.binding as P
+
+    for kw in ({"chunk_rows": 3}, {"chunk_rows": 128}, {"n_dispatchers": 9}, {"ring_slots": 100}, {"ring_slots": 8192}):
+        with pytest.raises(P.AesOffError) as e:
+            P.aes_engine_start(0, **kw)
+        assert e.value.code == P.AES_E_INVAL, kw
+
+
 def test_product_does_not_touch_oracle():
     """The product path must not route through oracle/ (that would void parity)."""
     pkg = os.path.join(ROOT, "paper_2607_02630_b200")
