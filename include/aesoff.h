@@ -20,7 +20,7 @@
  *
  * Conventions common to all calls
  *   - Plain C types only.  "host" / "device" is stated for every pointer.
- *   - One engine per process (one process per GPU).  All calls are thread-safe
+ *   - One engine per GPU, up to 8 per process (one process per GPU works as well).  All calls are thread-safe
  *     unless stated; aes_ctr_submit() may be called from many executor threads
  *     ("worker pool", "32-thread executor").
  *   - Errors are negative ints (AES_E_*); a call that returns NULL / 0 leaves
@@ -136,8 +136,26 @@ typedef struct aes_engine_info {
                                     1/8-row units, ...                                */
     uint64_t cut_halves;         /* ... into half rows, ...                           */
     uint64_t cut_rows;           /* ... into whole rows (see fine_rows above)         */
+    uint32_t engines_running;    /* engines of this process that accept requests      */
+    uint32_t reserved1;
 } aes_engine_info_t;
-int aes_engine_info(aes_engine_info_t *out);     /* host pointer; AES_OK / AES_E_INVAL */
+int aes_engine_info(aes_engine_info_t *out);     /* host pointer; AES_OK / AES_E_INVAL.  The running
+                                                    engine on the lowest device (else the last one run) */
+int aes_engine_info_device(int device, aes_engine_info_t *out);
+
+/* ---- several GPUs: one engine each, and a router ----------------
+ * Requests are independent ("each offload belongs to one request"), so the path
+ * shards over the GPUs of a node with NO exchange step: aes_engine_start() may be called once per device
+ * (up to 8 per process), and aes_ctr_submit() sends each request to the engine of the GPU that owns its
+ * dst, else its src (cudaPointerGetAttributes, remembered per 2 MiB page and per thread); requests whose
+ * src and dst are both host memory go round the running engines.  A request whose memory belongs to a GPU
+ * without a running engine fails with AES_E_STOPPED.  With one engine running nothing is looked up.  A
+ * handle carries its engine in its top byte; aes_poll / aes_wait take handles of any engine.  A context
+ * may be used on all engines (its key is filed per engine).  NVLink is not used, no collective runs.
+ * aes_engine_stop() stops every running engine, aes_engine_stop_device() one.  aes_route_flush() forgets
+ * the remembered owners: call it after device memory has been freed and its addresses handed to another GPU. */
+int  aes_engine_stop_device(int device);
+void aes_route_flush(void);
 
 /* ---- key expansion (step a1; FIPS-197 sec. 5.2) -----------------------------
  * key: host pointer to keybits/8 bytes, copied.  keybits in {128, 192, 256} (BASELINE.json

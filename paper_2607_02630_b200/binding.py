@@ -51,7 +51,8 @@ class aes_engine_info_t(ctypes.Structure):
                 ("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32),
                 ("smem_bytes_per_cta", ctypes.c_uint32), ("n_dispatchers", ctypes.c_uint32),
                 ("submitted", ctypes.c_uint64), ("completed", ctypes.c_uint64), ("kernel_launches", ctypes.c_uint64),
-                ("cut_eighths", ctypes.c_uint64), ("cut_halves", ctypes.c_uint64), ("cut_rows", ctypes.c_uint64)]
+                ("cut_eighths", ctypes.c_uint64), ("cut_halves", ctypes.c_uint64), ("cut_rows", ctypes.c_uint64),
+                ("engines_running", ctypes.c_uint32), ("reserved1", ctypes.c_uint32)]
 
 
 class aes_calib_t(ctypes.Structure):
@@ -83,6 +84,9 @@ def _load() -> ctypes.CDLL:
         "aes_engine_start": (i32, [i32, vp]),
         "aes_engine_stop": (i32, []),
         "aes_engine_info": (i32, [vp]),
+        "aes_engine_info_device": (i32, [i32, vp]),
+        "aes_engine_stop_device": (i32, [i32]),
+        "aes_route_flush": (None, []),
         "aes_ctx_create": (vp, [vp, i32]),
         "aes_ctx_destroy": (None, [vp]),
         "aes_ctx_round_keys": (i32, [vp, vp]),
@@ -107,7 +111,7 @@ def _load() -> ctypes.CDLL:
 
 
 _lib = _load()
-EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_ctx_create", "aes_ctx_destroy",
+EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_engine_info_device", "aes_engine_stop_device", "aes_route_flush", "aes_ctx_create", "aes_ctx_destroy",
            "aes_ctx_round_keys", "aes_ctr_submit", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
            "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run", "aes_loop_run_mt", "aes_openloop_run", "aes_calibrate")
 
@@ -136,10 +140,21 @@ def aes_engine_stop() -> None:
     _check(_lib.aes_engine_stop(), "aes_engine_stop")
 
 
-def aes_engine_info() -> dict:
+def aes_engine_stop_device(device: int) -> None:
+    _check(_lib.aes_engine_stop_device(device), "aes_engine_stop_device")
+
+
+def aes_route_flush() -> None:
+    _lib.aes_route_flush()
+
+
+def aes_engine_info(device: int | None = None) -> dict:
     info = aes_engine_info_t()
-    _check(_lib.aes_engine_info(ctypes.byref(info)), "aes_engine_info")
-    return {k: getattr(info, k) for k, _ in aes_engine_info_t._fields_}
+    if device is None:
+        _check(_lib.aes_engine_info(ctypes.byref(info)), "aes_engine_info")
+    else:
+        _check(_lib.aes_engine_info_device(device, ctypes.byref(info)), "aes_engine_info_device")
+    return {k: getattr(info, k) for k, _ in aes_engine_info_t._fields_ if k != "reserved1"}
 
 
 # ---- contexts ---------------------------------------------------------------------------------

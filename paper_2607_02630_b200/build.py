@@ -17,7 +17,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 SO = os.path.join(_PKG, "libaesoff.so")
-SOURCES = ["aesoff_kernels.cu", "aesoff_calib.cu", "aesoff_runtime.cpp", "aesoff_keys.cpp"]
+SOURCES = ["aesoff_kernels.cu", "aesoff_calib.cu", "aesoff_runtime.cpp", "aesoff_keys.cpp", "aesoff_router.cpp"]
 HEADERS = ["aesoff_shared.h", "aesoff_internal.h", "aesoff_cipher.cuh", os.path.join(_ROOT, "include", "aesoff.h")]
 
 NVCC_FLAGS = [

@@ -18,17 +18,33 @@
 #define AESOFF_CTX_INSTALLING 2u
 #define AESOFF_CTX_INSTALLED  3u
 
+#define AESOFF_MAX_DEVICES 8 /* engines per process: one per GPU of a node */
+
+/* where a context's key is on ONE engine (each GPU has its own key table) */
+struct aes_ctx_dev {
+    uint32_t state;       /* AESOFF_CTX_*, accessed atomically */
+    uint32_t id;          /* ktab index once state >= INSTALLING */
+    uint64_t epoch;       /* ktab generation the id belongs to */
+    uint64_t install_seq; /* sequence number of the request that installs the key (0 = not claimed yet) */
+};
+
 struct aes_ctx {
     uint32_t rk[60]; /* round keys as little-endian-loaded words, zero padded (host expansion) */
     int32_t nr;      /* 10, 12 or 14 */
     int32_t keybits;
     uint32_t key[8]; /* the cipher key as little-endian-loaded words, zero padded */
-    uint32_t state;  /* AESOFF_CTX_*, accessed atomically */
-    uint32_t id;     /* ktab index once state >= INSTALLING */
-    uint64_t epoch;  /* ktab generation the id belongs to */
-    uint64_t install_seq; /* sequence number of the request that installs the key (0 = not claimed yet) */
     uint32_t rk_ready; /* rk[] has been filled (lazily: the engine path expands keys on the device) */
+    uint32_t pad_;
+    aes_ctx_dev dev[AESOFF_MAX_DEVICES];
 };
+
+/* Which engine a request goes to (aesoff_router.cpp; "requests routed to the GPU that owns
+ * their src/dst").  owner: device index of the memory, AESOFF_OWNER_HOST for host memory.                        */
+#define AESOFF_OWNER_HOST (-2)
+int aesoff_route_decide(int src_owner, int dst_owner, uint32_t running_mask, uint32_t *round_robin);
+typedef int (*aesoff_owner_fn)(const void *ptr); /* resolves the owner of an address (cudaPointerGetAttributes) */
+int aesoff_route_owner_cached(const void *ptr, aesoff_owner_fn resolve);
+void aesoff_route_flush_cache(void);
 
 const uint32_t *aesoff_T0_table();
 int aesoff_key_expand(const uint8_t *key, int keybits, uint32_t rk[60]);

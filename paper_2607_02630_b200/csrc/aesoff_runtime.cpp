@@ -114,8 +114,52 @@ struct Engine {
     bool broken = false;                  /* a CUDA call failed: rebuild everything at the next start */
 };
 
-Engine g_eng;
+/* One engine per GPU (requests shard over the GPUs of a node with no exchange
+ * step); a handle carries its engine's device index in its top byte, the sequence number below.          */
+Engine g_engs[AESOFF_MAX_DEVICES];
+std::atomic<uint32_t> g_running_mask{0}; /* bit d: the engine on device d accepts requests                */
+std::atomic<int> g_single{-1};           /* the device index if exactly one engine runs, else -1          */
+std::atomic<uint32_t> g_round_robin{0};
 std::mutex g_lifecycle;
+constexpr int HANDLE_DEV_SHIFT = 56;
+constexpr uint64_t HANDLE_SEQ_MASK = (1ull << HANDLE_DEV_SHIFT) - 1;
+
+void publish_running(int device, bool on)
+{
+    uint32_t m = g_running_mask.load();
+    m = on ? (m | (1u << device)) : (m & ~(1u << device));
+    g_running_mask.store(m, std::memory_order_release);
+    g_single.store(__builtin_popcount(m) == 1 ? __builtin_ctz(m) : -1, std::memory_order_release);
+}
+
+/* the owner of an address for the router: a device index, or AESOFF_OWNER_HOST */
+int resolve_owner(const void *ptr)
+{
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, ptr) != cudaSuccess) {
+        cudaGetLastError();
+        return AESOFF_OWNER_HOST;
+    }
+    return a.type == cudaMemoryTypeDevice ? a.device : AESOFF_OWNER_HOST;
+}
+
+/* the engine a request goes to, or nullptr (none running / the owner of its memory runs none) */
+Engine *route(const void *src, void *dst, size_t len)
+{
+    const int single = g_single.load(std::memory_order_acquire);
+    if (single >= 0) return &g_engs[single];
+    const uint32_t mask = g_running_mask.load(std::memory_order_acquire);
+    if (mask == 0) return nullptr;
+    int so = AESOFF_OWNER_HOST, dO = AESOFF_OWNER_HOST;
+    if (len) {
+        dO = aesoff_route_owner_cached(dst, resolve_owner);
+        if (dO < 0) so = aesoff_route_owner_cached(src, resolve_owner);
+    }
+    uint32_t rr = g_round_robin.load(std::memory_order_relaxed);
+    const int d = aesoff_route_decide(so, dO, mask, &rr);
+    if (so < 0 && dO < 0) g_round_robin.store(rr, std::memory_order_relaxed);
+    return d >= 0 ? &g_engs[d] : nullptr;
+}
 std::atomic<uint64_t> g_kernel_launches{0};
 
 inline bool engine_dead(const Engine &e)
@@ -253,21 +297,26 @@ extern "C" aes_ctx_t *aes_ctx_create(const uint8_t *key, int keybits)
     for (int i = 0; i < keybits / 32; ++i)
         c->key[i] = (uint32_t)key[4 * i] | ((uint32_t)key[4 * i + 1] << 8) | ((uint32_t)key[4 * i + 2] << 16) |
                     ((uint32_t)key[4 * i + 3] << 24);
-    c->state = AESOFF_CTX_FRESH;
-    c->id = AESOFF_KEY_NONE;
-    c->epoch = 0;
-    c->install_seq = 0;
+    for (int d = 0; d < AESOFF_MAX_DEVICES; ++d) {
+        c->dev[d].state = AESOFF_CTX_FRESH;
+        c->dev[d].id = AESOFF_KEY_NONE;
+        c->dev[d].epoch = 0;
+        c->dev[d].install_seq = 0;
+    }
     return c;
 }
 
 extern "C" void aes_ctx_destroy(aes_ctx_t *ctx)
 {
     if (!ctx) return;
-    if (__atomic_load_n(&ctx->state, __ATOMIC_ACQUIRE) >= AESOFF_CTX_INSTALLING && ctx->id != AESOFF_KEY_NONE) {
-        Engine &e = g_eng;
-        std::lock_guard<std::mutex> lk(e.id_mu);
-        /* requests in flight may still name the index: it rests until they must have completed */
-        if (ctx->epoch == e.k_epoch.load()) e.id_free.emplace_back(ctx->id, e.next_seq.load());
+    for (int d = 0; d < AESOFF_MAX_DEVICES; ++d) {
+        aes_ctx_dev &k = ctx->dev[d];
+        if (__atomic_load_n(&k.state, __ATOMIC_ACQUIRE) >= AESOFF_CTX_INSTALLING && k.id != AESOFF_KEY_NONE) {
+            Engine &e = g_engs[d];
+            std::lock_guard<std::mutex> lk(e.id_mu);
+            /* requests in flight may still name the index: it rests until they must have completed */
+            if (k.epoch == e.k_epoch.load()) e.id_free.emplace_back(k.id, e.next_seq.load());
+        }
     }
     explicit_bzero(ctx, sizeof(*ctx)); /* key hygiene: raw key and round keys do not outlive the context */
     free(ctx);
@@ -314,7 +363,8 @@ extern "C" int aes_ctx_round_keys(const aes_ctx_t *ctx_in, uint8_t *out)
 extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
 {
     std::lock_guard<std::mutex> lk(g_lifecycle);
-    Engine &e = g_eng;
+    if (device < 0 || device >= AESOFF_MAX_DEVICES) return fail(AES_E_CUDA);
+    Engine &e = g_engs[device];
     if (e.running.load()) return fail(AES_E_BUSY);
 
     aes_engine_opts_t o;
@@ -456,15 +506,17 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
         return fail(AES_E_STOPPED);
     }
     e.running.store(1, std::memory_order_release);
+    publish_running(device, true);
     return AES_OK;
 }
 
-extern "C" int aes_engine_stop(void)
+namespace {
+/* g_lifecycle held */
+int stop_engine(Engine &e)
 {
-    std::lock_guard<std::mutex> lk(g_lifecycle);
-    Engine &e = g_eng;
     if (!e.running.load()) return fail(AES_E_STOPPED);
     /* no new submissions from here on; the ones that passed their `running` check finish publishing */
+    publish_running(e.device, false);
     e.running.store(2, std::memory_order_seq_cst);
     for (int i = 0; i < SUBMIT_SHARDS; ++i)
         while (e.submitters[i].n.load(std::memory_order_seq_cst) != 0) CPU_RELAX();
@@ -503,12 +555,34 @@ extern "C" int aes_engine_stop(void)
     if (rc != AES_OK) return fail(rc);
     return AES_OK;
 }
+} /* namespace */
 
-extern "C" int aes_engine_info(aes_engine_info_t *out)
+extern "C" int aes_engine_stop_device(int device)
 {
-    if (!out) return fail(AES_E_INVAL);
+    std::lock_guard<std::mutex> lk(g_lifecycle);
+    if (device < 0 || device >= AESOFF_MAX_DEVICES) return fail(AES_E_INVAL);
+    return stop_engine(g_engs[device]);
+}
+
+extern "C" int aes_engine_stop(void)
+{
+    std::lock_guard<std::mutex> lk(g_lifecycle);
+    int rc = AES_E_STOPPED, n = 0;
+    for (int d = 0; d < AESOFF_MAX_DEVICES; ++d)
+        if (g_engs[d].running.load()) {
+            const int r = stop_engine(g_engs[d]);
+            if (n++ == 0 || r != AES_OK) rc = r;
+        }
+    if (rc != AES_OK) return fail(rc);
+    return AES_OK;
+}
+
+extern "C" int aes_engine_info_device(int device, aes_engine_info_t *out)
+{
+    if (!out || device < 0 || device >= AESOFF_MAX_DEVICES) return fail(AES_E_INVAL);
     memset(out, 0, sizeof(*out));
-    Engine &e = g_eng;
+    Engine &e = g_engs[device];
+    out->engines_running = (uint32_t)__builtin_popcount(g_running_mask.load());
     out->running = e.running.load() == 1 && e.hctl && !engine_dead(e);
     out->device = e.device;
     out->sm_count = e.sm_count;
@@ -539,11 +613,28 @@ extern "C" int aes_engine_info(aes_engine_info_t *out)
     return AES_OK;
 }
 
+/* the running engine on the lowest device; if none runs, the one that ran last on the lowest device */
+extern "C" int aes_engine_info(aes_engine_info_t *out)
+{
+    int pick = 0;
+    const uint32_t m = g_running_mask.load();
+    if (m) {
+        pick = __builtin_ctz(m);
+    } else {
+        for (int d = 0; d < AESOFF_MAX_DEVICES; ++d)
+            if (g_engs[d].device >= 0) {
+                pick = d;
+                break;
+            }
+    }
+    return aes_engine_info_device(pick, out);
+}
+
 /* AESOFF_DISP_STATS builds: per-dispatcher counters (polls that took requests, requests, token wait and work
  * in units of 64 ns, empty polls), 5 words per dispatcher; zeros otherwise.  Tuning aid, not in aesoff.h.   */
 extern "C" __attribute__((visibility("default"))) int aesoff_debug_dispatch_stats(uint32_t out[5 * AESOFF_MAX_DISPATCHERS])
 {
-    Engine &e = g_eng;
+    Engine &e = g_engs[g_single.load() >= 0 ? g_single.load() : 0];
     if (!e.hctl) return -1;
     for (uint32_t d = 0; d < AESOFF_MAX_DISPATCHERS; ++d)
         for (int i = 0; i < 5; ++i)
@@ -557,7 +648,6 @@ extern "C" __attribute__((visibility("default"))) int aesoff_debug_dispatch_stat
 extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], const void *src, void *dst,
                                        size_t len)
 {
-    Engine &e = g_eng;
     if (!ctx || !nonce) {
         fail(AES_E_INVAL);
         return 0;
@@ -567,6 +657,13 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
         fail(rc);
         return 0;
     }
+    Engine *ep = route(src, dst, len);
+    if (!ep) {
+        fail(AES_E_STOPPED);
+        return 0;
+    }
+    Engine &e = *ep;
+    aes_ctx_dev &ck = ctx->dev[e.device];
     /* counted BEFORE the running check: aes_engine_stop sets running = 2 and then waits for the count to
      * drop to 0, so a submit either fails here or has published its slot before the drain reads next_seq */
     struct InFlight {
@@ -583,29 +680,29 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
      * batches of requests side by side, so a lower sequence number alone does not mean "expanded first". */
     uint32_t kw = ((uint32_t)ctx->nr << 24) | AESOFF_KEY_NONE | AESOFF_KW_RAW;
     bool installing = false;
-    uint32_t st = __atomic_load_n(&ctx->state, __ATOMIC_ACQUIRE);
+    uint32_t st = __atomic_load_n(&ck.state, __ATOMIC_ACQUIRE);
     const uint64_t epoch_now = e.k_epoch.load(std::memory_order_acquire);
-    const bool epoch_ok = __atomic_load_n(&ctx->epoch, __ATOMIC_ACQUIRE) == epoch_now;
+    const bool epoch_ok = __atomic_load_n(&ck.epoch, __ATOMIC_ACQUIRE) == epoch_now;
     if (st == AESOFF_CTX_INSTALLING && epoch_ok) {
-        const uint64_t is = __atomic_load_n(&ctx->install_seq, __ATOMIC_ACQUIRE);
+        const uint64_t is = __atomic_load_n(&ck.install_seq, __ATOMIC_ACQUIRE);
         if (is != 0 && __atomic_load_n(&e.hmail[(is - 1) & e.Rm], __ATOMIC_ACQUIRE) >= is) {
-            __atomic_store_n(&ctx->state, AESOFF_CTX_INSTALLED, __ATOMIC_RELEASE);
+            __atomic_store_n(&ck.state, AESOFF_CTX_INSTALLED, __ATOMIC_RELEASE);
             st = AESOFF_CTX_INSTALLED;
         }
     }
     if (st == AESOFF_CTX_INSTALLED && epoch_ok) {
-        kw = ((uint32_t)ctx->nr << 24) | ctx->id;
+        kw = ((uint32_t)ctx->nr << 24) | ck.id;
     } else if (st == AESOFF_CTX_FRESH) {
-        __atomic_compare_exchange_n(&ctx->state, &st, AESOFF_CTX_SEEN, false, __ATOMIC_ACQ_REL, __ATOMIC_ACQUIRE);
+        __atomic_compare_exchange_n(&ck.state, &st, AESOFF_CTX_SEEN, false, __ATOMIC_ACQ_REL, __ATOMIC_ACQUIRE);
     } else if (st == AESOFF_CTX_SEEN || (st == AESOFF_CTX_INSTALLED && !epoch_ok)) {
         /* INSTALLED under an older ktab generation (the engine was rebuilt): install again */
         const uint32_t id = alloc_key_id(e);
         if (id != AESOFF_KEY_NONE) {
-            if (__atomic_compare_exchange_n(&ctx->state, &st, AESOFF_CTX_INSTALLING, false, __ATOMIC_ACQ_REL,
+            if (__atomic_compare_exchange_n(&ck.state, &st, AESOFF_CTX_INSTALLING, false, __ATOMIC_ACQ_REL,
                                             __ATOMIC_ACQUIRE)) {
-                __atomic_store_n(&ctx->install_seq, 0ull, __ATOMIC_RELEASE);
-                ctx->id = id;
-                __atomic_store_n(&ctx->epoch, epoch_now, __ATOMIC_RELEASE);
+                __atomic_store_n(&ck.install_seq, 0ull, __ATOMIC_RELEASE);
+                ck.id = id;
+                __atomic_store_n(&ck.epoch, epoch_now, __ATOMIC_RELEASE);
                 kw |= AESOFF_KW_INSTALL;
                 kw = (kw & ~0xffffu) | id;
                 installing = true;
@@ -623,11 +720,11 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
             if (installing) { /* undo: the index was never named by a descriptor */
                 {
                     std::lock_guard<std::mutex> lk(e.id_mu);
-                    e.id_free.emplace_front(ctx->id, 0ull);
+                    e.id_free.emplace_front(ck.id, 0ull);
                 }
-                ctx->id = AESOFF_KEY_NONE;
-                __atomic_store_n(&ctx->epoch, 0ull, __ATOMIC_RELEASE);
-                __atomic_store_n(&ctx->state, AESOFF_CTX_SEEN, __ATOMIC_RELEASE);
+                ck.id = AESOFF_KEY_NONE;
+                __atomic_store_n(&ck.epoch, 0ull, __ATOMIC_RELEASE);
+                __atomic_store_n(&ck.state, AESOFF_CTX_SEEN, __ATOMIC_RELEASE);
             }
             fail(AES_E_AGAIN);
             return 0;
@@ -658,20 +755,23 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
     store_piece(w + 8, (uint32_t)a_dst, (uint32_t)(a_dst >> 32), (uint32_t)a_len, tag);
     store_piece(w + 12, (uint32_t)(a_len >> 32), kw, 0u, tag);
     /* later submits name ktab[id] once this request, which fills it, has completed */
-    if (installing) __atomic_store_n(&ctx->install_seq, s, __ATOMIC_RELEASE);
-    return (aes_handle_t)s;
+    if (installing) __atomic_store_n(&ck.install_seq, s, __ATOMIC_RELEASE);
+    return (aes_handle_t)(s | ((uint64_t)e.device << HANDLE_DEV_SHIFT));
 }
 
 extern "C" int aes_poll(aes_handle_t h)
 {
-    Engine &e = g_eng;
-    /* A valid handle is below next_seq.  That word is claimed by every submit of every thread, so a poll does
-     * not read it: it compares with this thread's last copy and refreshes the copy only for a handle above it. */
-    thread_local uint64_t seen_next = 0;
+    /* A valid handle is below its engine's next_seq.  That word is claimed by every submit of every thread, so a
+     * poll does not read it: it compares with this thread's last copy and refreshes the copy only for a handle above it. */
+    thread_local uint64_t seen_next[AESOFF_MAX_DEVICES] = {0};
+    const unsigned dev = (unsigned)(h >> HANDLE_DEV_SHIFT);
+    if (dev >= AESOFF_MAX_DEVICES) return fail(AES_E_INVAL);
+    Engine &e = g_engs[dev];
+    h &= HANDLE_SEQ_MASK;
     if (h == 0) return fail(AES_E_INVAL);
-    if (h >= seen_next) {
-        seen_next = e.next_seq.load(std::memory_order_acquire);
-        if (h >= seen_next) return fail(AES_E_INVAL);
+    if (h >= seen_next[dev]) {
+        seen_next[dev] = e.next_seq.load(std::memory_order_acquire);
+        if (h >= seen_next[dev]) return fail(AES_E_INVAL);
     }
     if (h < e.done_upto.load(std::memory_order_acquire)) {
         /* a run that has been stopped: a clean stop drained everything, an unclean one lists what it lost */
@@ -717,6 +817,8 @@ extern "C" int aes_wait(aes_handle_t h, uint64_t timeout_ns)
         }
     }
 }
+
+extern "C" void aes_route_flush(void) { aesoff_route_flush_cache(); }
 
 /* ============================================================================================ */
 /* pinned host memory                                                                            */
@@ -779,7 +881,7 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     if (!ctxs || !nonces || !srcs || !dsts || !lens) return fail(AES_E_INVAL);
     if (chunk_rows == 0) chunk_rows = 4;
     if (chunk_rows > 64) return fail(AES_E_INVAL);
-    if (g_eng.running.load()) return fail(AES_E_BUSY);
+    if (device >= 0 && device < AESOFF_MAX_DEVICES && g_engs[device].running.load()) return fail(AES_E_BUSY);
     for (size_t i = 0; i < n; ++i) {
         if (!ctxs[i]) return fail(AES_E_INVAL);
         const int rc = check_buffers(srcs[i], dsts[i], lens[i]);
@@ -1007,11 +1109,14 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
     if (!spec->keys && !spec->ctx) return fail(AES_E_INVAL);
     if (spec->keys && !spec->keybits) return fail(AES_E_INVAL);
     if (spec->n == 0 || spec->window == 0) return fail(AES_E_INVAL);
-    Engine &e = g_eng;
-    if (e.running.load() != 1) return fail(AES_E_STOPPED);
+    const uint32_t running = g_running_mask.load(std::memory_order_acquire);
+    if (!running) return fail(AES_E_STOPPED);
+    uint32_t ring_total = 0; /* what can be in flight over all engines */
+    for (int d = 0; d < AESOFF_MAX_DEVICES; ++d)
+        if ((running >> d) & 1u) ring_total += g_engs[d].R;
     const uint64_t repeat = spec->repeat ? spec->repeat : 1;
     const uint64_t total = (uint64_t)spec->n * repeat;
-    const uint32_t window = spec->window > e.R ? e.R : spec->window;
+    const uint32_t window = spec->window > ring_total ? ring_total : spec->window;
     const double nspt = tick_ns();
 
     /* In flight, in submission order.  Completions come roughly in that order, so a sweep polls from the oldest
@@ -1088,7 +1193,7 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
 extern "C" int aes_calibrate(int device, aes_calib_t *out)
 {
     if (!out) return fail(AES_E_INVAL);
-    if (g_eng.running.load()) return fail(AES_E_BUSY);
+    if (device >= 0 && device < AESOFF_MAX_DEVICES && g_engs[device].running.load()) return fail(AES_E_BUSY);
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(AES_E_CUDA);
     double v[6];
@@ -1112,15 +1217,14 @@ extern "C" int aes_openloop_run(const aes_loop_spec_t *spec, const uint64_t *arr
     if (!spec || !res || !arrival_ns || !spec->ctx || !spec->nonces || !spec->srcs || !spec->dsts || !spec->lens)
         return fail(AES_E_INVAL);
     if (spec->n == 0) return fail(AES_E_INVAL);
-    Engine &e = g_eng;
-    if (e.running.load() != 1) return fail(AES_E_STOPPED);
+    if (!g_running_mask.load(std::memory_order_acquire)) return fail(AES_E_STOPPED);
     const size_t n = spec->n;
     struct Fly {
         aes_handle_t h;
         size_t index;
     };
     std::vector<Fly> fly;
-    fly.reserve(e.R);
+    fly.reserve(4096);
     memset(res, 0, sizeof(*res));
     size_t next = 0, done = 0;
     uint64_t bytes = 0;

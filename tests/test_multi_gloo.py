@@ -52,3 +52,40 @@ def test_single_process_passthrough():
 
     value, ms = multi.job_throughput(4.0, 8 * 10**9)
     assert ms == 4.0 and value == pytest.approx(2e12)
+
+
+def test_bench_rank_logic_two_ranks_on_gloo():
+    """bench.py's own N-rank logic, launched the way the driver launches it (torch.distributed.run, one rank per
+    GPU), with the GPU work left out: rank 0 prints n_gpus == 2, the max over ranks and the summed bytes."""
+    import json
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(_free_port()), os.path.join(root, "bench.py"), "--gpus", "2", "--plumbing-check"]
+    p = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=root)
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [json.loads(ln) for ln in p.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, p.stdout
+    d = lines[0]
+    assert d["n_gpus"] == 2 and d["ms_max"] == pytest.approx(11.0) and d["value"] == pytest.approx(2.0 / 11e-3)
+
+
+def test_bench_refuses_a_rank_count_that_is_not_gpus():
+    """--gpus 4 under a 1-rank launch (or on a node with fewer GPUs) must fail loudly, not print n_gpus: 1."""
+    import subprocess
+    import sys
+
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    p = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "4", "--plumbing-check"], capture_output=True,
+                       text=True, timeout=120, cwd=root, env=env)
+    assert p.returncode != 0 and "n_gpus would lie" in (p.stderr + p.stdout)
+    import torch
+
+    if torch.cuda.device_count() < 4:
+        env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+        p = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "4", "--steps", "1"], capture_output=True,
+                           text=True, timeout=120, cwd=root, env=env)
+        assert p.returncode != 0 and "GPU(s)" in (p.stderr + p.stdout)
