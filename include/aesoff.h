@@ -199,6 +199,20 @@ int aes_ctx_round_keys(const aes_ctx_t *ctx, uint8_t *out);
 aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16],
                             const void *src, void *dst, size_t len);
 
+/* ---- other modes on the same engine ------------------------------------
+ * "The GPU path performs AES" with the mode unstated; BASELINE.json fixes CTR for the headline, and
+ * the two other modes whose blocks are independent -- so that they spread over warps exactly like CTR -- ride the
+ * same ring, units and completion path:
+ *   aes_ecb_submit          SP 800-38A sec. 6.1: C_j = Cipher_K(P_j), or with decrypt != 0 P_j = InvCipher_K(C_j)
+ *   aes_cbc_decrypt_submit  SP 800-38A sec. 6.2: P_j = InvCipher_K(C_j) xor C_{j-1}, C_0 = iv (host, 16 bytes, copied)
+ * (CBC encryption chains every block on the one before it: no data parallelism, not offered.)  Arguments as for
+ * aes_ctr_submit, and: len must be a multiple of 16 (AES_E_INVAL; these modes have no partial block, padding is the
+ * caller's); for CBC dst must not be src (AES_E_OVERLAP): a block's predecessor is read by another warp, which must
+ * find ciphertext there.  Decryption runs the equivalent inverse cipher (FIPS-197 sec. 5.3.5) out of one more
+ * table; it is bound by the ALU pipe at about half the CTR rate.                                       */
+aes_handle_t aes_ecb_submit(aes_ctx_t *ctx, int decrypt, const void *src, void *dst, size_t len);
+aes_handle_t aes_cbc_decrypt_submit(aes_ctx_t *ctx, const uint8_t iv[16], const void *src, void *dst, size_t len);
+
 /* ---- completion (step a7) ----------------------------------------------------
  * aes_poll: 1 = complete, 0 = pending, < 0 = error (AES_E_INVAL for a handle that
  * was never issued, AES_E_STOPPED if the engine died with the request pending).
@@ -231,6 +245,17 @@ int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonces,
                          const void *const *srcs, void *const *dsts,
                          const size_t *lens, size_t n,
                          int device, void *cuda_stream, uint32_t chunk_rows);
+
+/* The same with a mode per request (modes == NULL: all CTR); nonces[16 i ..] is the ICB (CTR), the IV (CBC) or
+ * ignored (ECB).  Restrictions of the modes as above.                                                              */
+#define AES_MODE_CTR     0
+#define AES_MODE_ECB_ENC 1
+#define AES_MODE_ECB_DEC 2
+#define AES_MODE_CBC_DEC 3
+int aes_mode_launch_batch(const int32_t *modes, aes_ctx_t *const *ctxs, const uint8_t *nonces,
+                          const void *const *srcs, void *const *dsts,
+                          const size_t *lens, size_t n,
+                          int device, void *cuda_stream, uint32_t chunk_rows);
 
 /* ---- pinned host memory the GPU can address (for host-resident payloads) ----- */
 void *aes_host_alloc(size_t bytes);        /* NULL on error (AES_E_CUDA / AES_E_NOMEM) */

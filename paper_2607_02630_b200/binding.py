@@ -91,6 +91,9 @@ def _load() -> ctypes.CDLL:
         "aes_ctx_destroy": (None, [vp]),
         "aes_ctx_round_keys": (i32, [vp, vp]),
         "aes_ctr_submit": (u64, [vp, vp, vp, vp, sz]),
+        "aes_ecb_submit": (u64, [vp, i32, vp, vp, sz]),
+        "aes_cbc_decrypt_submit": (u64, [vp, vp, vp, vp, sz]),
+        "aes_mode_launch_batch": (i32, [vp, vp, vp, vp, vp, vp, sz, i32, vp, ctypes.c_uint32]),
         "aes_poll": (i32, [u64]),
         "aes_wait": (i32, [u64, u64]),
         "aes_last_error": (i32, []),
@@ -112,7 +115,7 @@ def _load() -> ctypes.CDLL:
 
 _lib = _load()
 EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_engine_info_device", "aes_engine_stop_device", "aes_route_flush", "aes_ctx_create", "aes_ctx_destroy",
-           "aes_ctx_round_keys", "aes_ctr_submit", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
+           "aes_ctx_round_keys", "aes_ctr_submit", "aes_ecb_submit", "aes_cbc_decrypt_submit", "aes_mode_launch_batch", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
            "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run", "aes_loop_run_mt", "aes_openloop_run", "aes_calibrate")
 
 
@@ -187,6 +190,20 @@ def aes_ctr_submit(ctx: int, nonce: bytes, src: int, dst: int, length: int) -> i
     return h
 
 
+def aes_ecb_submit(ctx: int, decrypt: bool, src: int, dst: int, length: int) -> int:
+    h = _lib.aes_ecb_submit(ctx, 1 if decrypt else 0, src, dst, length)
+    if h == 0:
+        raise AesOffError(aes_last_error(), "aes_ecb_submit")
+    return h
+
+
+def aes_cbc_decrypt_submit(ctx: int, iv: bytes, src: int, dst: int, length: int) -> int:
+    h = _lib.aes_cbc_decrypt_submit(ctx, bytes(iv), src, dst, length)
+    if h == 0:
+        raise AesOffError(aes_last_error(), "aes_cbc_decrypt_submit")
+    return h
+
+
 def aes_poll(handle: int) -> bool:
     r = _lib.aes_poll(handle)
     if r < 0:
@@ -213,6 +230,23 @@ def aes_ctr_launch_batch(ctxs, nonces, srcs, dsts, lens, device: int = 0, cuda_s
     assert a_non.size == 16 * n and a_ctx.size == n and a_src.size == n and a_dst.size == n
     _check(_lib.aes_ctr_launch_batch(a_ctx.ctypes.data, a_non.ctypes.data, a_src.ctypes.data, a_dst.ctypes.data,
                                      a_len.ctypes.data, n, device, cuda_stream, chunk_rows), "aes_ctr_launch_batch")
+
+
+AES_MODE_CTR, AES_MODE_ECB_ENC, AES_MODE_ECB_DEC, AES_MODE_CBC_DEC = 0, 1, 2, 3
+
+
+def aes_mode_launch_batch(modes, ctxs, nonces, srcs, dsts, lens, device: int = 0, cuda_stream: int = 0,
+                          chunk_rows: int = 0) -> None:
+    """aes_ctr_launch_batch with a mode per request (AES_MODE_*); nonces: n x 16 bytes (ICB / IV / ignored)."""
+    n = len(lens)
+    a_mode = np.ascontiguousarray(np.asarray(modes, dtype=np.int32))
+    a_ctx, a_src, a_dst, a_len = _ptr_array(ctxs), _ptr_array(srcs), _ptr_array(dsts), _ptr_array(lens)
+    a_non = np.ascontiguousarray(np.frombuffer(bytes(nonces), dtype=np.uint8) if isinstance(nonces, (bytes, bytearray))
+                                 else np.asarray(nonces, dtype=np.uint8)).reshape(-1)
+    assert a_non.size == 16 * n and a_ctx.size == n and a_src.size == n and a_dst.size == n and a_mode.size == n
+    _check(_lib.aes_mode_launch_batch(a_mode.ctypes.data, a_ctx.ctypes.data, a_non.ctypes.data, a_src.ctypes.data,
+                                      a_dst.ctypes.data, a_len.ctypes.data, n, device, cuda_stream, chunk_rows),
+           "aes_mode_launch_batch")
 
 
 # ---- pinned host memory ---------------------------------------------------------------------------

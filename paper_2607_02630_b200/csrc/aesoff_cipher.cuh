@@ -38,6 +38,12 @@ constexpr int OFF_T1 = 128;
 constexpr int OFF_T2 = 65536;
 constexpr int OFF_T3 = 65536 + 128;
 constexpr uint32_t TABLE_BYTES = 131072;
+/* The decryption modes (ECB, CBC) run the equivalent inverse cipher (FIPS-197 sec. 5.3.5)
+ * out of ONE more table, Td0, again one replica per bank: entry x of lane l at TD_OFF + x * 128 + l * 4, 32 KiB
+ * behind the four encryption tables (all the shared memory an SM has left).  Td1..Td3 are byte rotations done in
+ * registers and the address needs a shift and a mask: these modes are bound by the ALU pipe, not by lookups.    */
+constexpr uint32_t TD_OFF = TABLE_BYTES;
+constexpr uint32_t TD_BYTES = 32768;
 
 template <int OFF>
 __device__ __forceinline__ uint32_t lds_off(uint32_t a)
@@ -103,6 +109,44 @@ __device__ __forceinline__ void fill_tables(uint32_t tbase, const uint32_t *T0, 
         sts(a + OFF_T3, rotl32(t0, 24));
     }
     fill_barrier(nthreads);
+}
+
+/* Td0 replicas (global table at Td0[0..255]); called like fill_tables, after it */
+__device__ __forceinline__ void fill_td(uint32_t tbase, const uint32_t *Td0, uint32_t tid, uint32_t nthreads)
+{
+    for (uint32_t idx = tid; idx < 256u * 32u; idx += nthreads) sts(tbase + TD_OFF + idx * 4u, __ldg(Td0 + (idx >> 5)));
+    fill_barrier(nthreads);
+}
+/* Td0[byte K of x] out of this lane's replica; ybd = (tbase + TD_OFF) | lane * 4 */
+template <int K>
+__device__ __forceinline__ uint32_t td(uint32_t x, uint32_t ybd)
+{
+    const uint32_t sh = (K == 0) ? (x << 7) : (x >> (8 * K - 7));
+    uint32_t v;
+    asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((sh & 0x7f80u) | ybd));
+    return v;
+}
+__device__ __forceinline__ uint32_t xor_bytes(uint32_t t) /* InvSubBytes(x) from Td0[x] */
+{
+    t ^= t >> 16;
+    return (t ^ (t >> 8)) & 0xffu;
+}
+/* one column of an inverse round: InvShiftRows moves row r right by r columns */
+__device__ __forceinline__ uint32_t td_col(uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t ybd)
+{
+    return td<0>(a, ybd) ^ rotl32(td<1>(b, ybd), 8) ^ rotl32(td<2>(c, ybd), 16) ^ rotl32(td<3>(d, ybd), 24);
+}
+__device__ __forceinline__ uint32_t tdlast_col(uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t ybd)
+{
+    return xor_bytes(td<0>(a, ybd)) | (xor_bytes(td<1>(b, ybd)) << 8) | (xor_bytes(td<2>(c, ybd)) << 16) |
+           (xor_bytes(td<3>(d, ybd)) << 24);
+}
+/* Round keys of the equivalent inverse cipher (sec. 5.3.5): dw[r] = InvMixColumns(w[r]) for 0 < r < Nr, word by word:
+ * InvMixColumns of a column is Td0[S[a0]] ^ rot(Td0[S[a1]]) ^ ..., S[a] being byte 1 of T0[a].                  */
+__device__ __forceinline__ uint32_t inv_mix_word(uint32_t w, uint32_t ybase, uint32_t ybd)
+{
+    const uint32_t s0 = TL(0, 0, w) >> 8, s1 = TL(0, 1, w) >> 8, s2 = TL(0, 2, w) >> 8, s3 = TL(0, 3, w) >> 8;
+    return td<0>(s0, ybd) ^ rotl32(td<0>(s1, ybd), 8) ^ rotl32(td<0>(s2, ybd), 16) ^ rotl32(td<0>(s3, ybd), 24);
 }
 
 /* ------------------------------------------------------------------------------------------ */
@@ -343,6 +387,116 @@ __device__ __forceinline__ void ctr_request_rows(uint32_t ybase, const uint4 *rk
             if (kb * 512u >= row_bytes) break;
             if ((kb + NB) * 32u <= lo_L) continue;
             row_blocks<NB>(rc, ybase, rk4, nr, src + row_off, dst + row_off, lo_L, row_bytes, lane, kb);
+        }
+    }
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* ECB and CBC-decrypt (SP 800-38A sec. 6.1, 6.2): whole blocks, no counter                     */
+/* ------------------------------------------------------------------------------------------ */
+/* NB blocks per lane of "row" m (4 KiB of the payload): block L = lane + 32 (kb + b) of the row.
+ * MODE: AESOFF_MODE_ECB_ENC  C_j = Cipher(P_j)          (encryption tables, all rounds in full)
+ *       AESOFF_MODE_ECB_DEC  P_j = InvCipher(C_j)       (rk4 holds the equivalent inverse cipher's keys)
+ *       AESOFF_MODE_CBC_DEC  P_j = InvCipher(C_j) ^ C_{j-1}, C_0 = IV; src and dst must not overlap, since the
+ *                            block before this lane's belongs to another lane, warp or CTA                      */
+template <int NB, int MODE>
+__device__ __forceinline__ void mode_blocks(uint32_t ybase, uint32_t ybd, const uint4 *rk4, int nr, const uint8_t *src_row,
+                                            uint8_t *dst_row, uint32_t row_bytes, bool first_row, uint4 iv, uint32_t lane,
+                                            uint32_t kb)
+{
+    uint32_t st[NB][4];
+    uint4 prev[NB];
+    bool live[NB];
+    const uint4 kin = rk4[MODE == AESOFF_MODE_ECB_ENC ? 0 : nr];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        const uint32_t off = (lane + 32u * (kb + b)) * 16u;
+        live[b] = off + 16u <= row_bytes;
+        uint4 p = make_uint4(0, 0, 0, 0);
+        prev[b] = iv;
+        if (live[b]) {
+            p = __ldcg(reinterpret_cast<const uint4 *>(src_row + off));
+            if (MODE == AESOFF_MODE_CBC_DEC && !(first_row && off == 0u))
+                prev[b] = __ldcg(reinterpret_cast<const uint4 *>(src_row + off) - 1);
+        }
+        st[b][0] = p.x ^ kin.x;
+        st[b][1] = p.y ^ kin.y;
+        st[b][2] = p.z ^ kin.z;
+        st[b][3] = p.w ^ kin.w;
+    }
+    if (MODE == AESOFF_MODE_ECB_ENC) {
+#pragma unroll 1
+        for (int r = 1; r < nr; ++r) {
+            const uint4 kk = rk4[r];
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const uint32_t x0 = st[b][0], x1 = st[b][1], x2 = st[b][2], x3 = st[b][3];
+                st[b][0] = TL(0, 0, x0) ^ TL(1, 1, x1) ^ TL(2, 2, x2) ^ TL(3, 3, x3) ^ kk.x;
+                st[b][1] = TL(0, 0, x1) ^ TL(1, 1, x2) ^ TL(2, 2, x3) ^ TL(3, 3, x0) ^ kk.y;
+                st[b][2] = TL(0, 0, x2) ^ TL(1, 1, x3) ^ TL(2, 2, x0) ^ TL(3, 3, x1) ^ kk.z;
+                st[b][3] = TL(0, 0, x3) ^ TL(1, 1, x0) ^ TL(2, 2, x1) ^ TL(3, 3, x2) ^ kk.w;
+            }
+        }
+    } else {
+#pragma unroll 1
+        for (int r = nr - 1; r > 0; --r) {
+            const uint4 kk = rk4[r];
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const uint32_t x0 = st[b][0], x1 = st[b][1], x2 = st[b][2], x3 = st[b][3];
+                st[b][0] = td_col(x0, x3, x2, x1, ybd) ^ kk.x;
+                st[b][1] = td_col(x1, x0, x3, x2, ybd) ^ kk.y;
+                st[b][2] = td_col(x2, x1, x0, x3, ybd) ^ kk.z;
+                st[b][3] = td_col(x3, x2, x1, x0, ybd) ^ kk.w;
+            }
+        }
+    }
+    const uint4 kk = rk4[MODE == AESOFF_MODE_ECB_ENC ? nr : 0];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        const uint32_t x0 = st[b][0], x1 = st[b][1], x2 = st[b][2], x3 = st[b][3];
+        uint4 o;
+        if (MODE == AESOFF_MODE_ECB_ENC) {
+            o.x = bitsel(bitsel(TL(3, 0, x0), TL(0, 1, x1), 0x000000ffu), bitsel(TL(0, 2, x2), TL(1, 3, x3), 0x00ff0000u), 0x0000ffffu) ^ kk.x;
+            o.y = bitsel(bitsel(TL(3, 0, x1), TL(0, 1, x2), 0x000000ffu), bitsel(TL(0, 2, x3), TL(1, 3, x0), 0x00ff0000u), 0x0000ffffu) ^ kk.y;
+            o.z = bitsel(bitsel(TL(3, 0, x2), TL(0, 1, x3), 0x000000ffu), bitsel(TL(0, 2, x0), TL(1, 3, x1), 0x00ff0000u), 0x0000ffffu) ^ kk.z;
+            o.w = bitsel(bitsel(TL(3, 0, x3), TL(0, 1, x0), 0x000000ffu), bitsel(TL(0, 2, x1), TL(1, 3, x2), 0x00ff0000u), 0x0000ffffu) ^ kk.w;
+        } else {
+            o.x = tdlast_col(x0, x3, x2, x1, ybd) ^ kk.x;
+            o.y = tdlast_col(x1, x0, x3, x2, ybd) ^ kk.y;
+            o.z = tdlast_col(x2, x1, x0, x3, ybd) ^ kk.z;
+            o.w = tdlast_col(x3, x2, x1, x0, ybd) ^ kk.w;
+            if (MODE == AESOFF_MODE_CBC_DEC) {
+                o.x ^= prev[b].x;
+                o.y ^= prev[b].y;
+                o.z ^= prev[b].z;
+                o.w ^= prev[b].w;
+            }
+        }
+        if (live[b]) __stcg(reinterpret_cast<uint4 *>(dst_row + (lane + 32u * (kb + b)) * 16u), o);
+    }
+}
+
+/* rows m0 .. m0 + count - 1 of a request in one of the block modes, k-iterations [kb0, kb1) of each */
+template <int NB>
+__device__ __noinline__ void mode_request_rows(uint32_t mode, uint32_t ybase, uint32_t ybd, const uint4 *rk4, int nr, uint4 iv,
+                                               const uint8_t *src, uint8_t *dst, uint64_t len, uint64_t m0, uint32_t count,
+                                               uint32_t lane, uint32_t kb0, uint32_t kb1)
+{
+#pragma unroll 1
+    for (uint32_t r = 0; r < count; ++r) {
+        const uint64_t m = m0 + r, row_off = m * AESOFF_ROW_BYTES;
+        if (row_off >= len) break;
+        const uint32_t row_bytes = len - row_off >= AESOFF_ROW_BYTES ? AESOFF_ROW_BYTES : (uint32_t)(len - row_off);
+#pragma unroll 1
+        for (uint32_t kb = kb0; kb < kb1; kb += NB) {
+            if (kb * 512u >= row_bytes) break;
+            if (mode == AESOFF_MODE_ECB_ENC)
+                mode_blocks<NB, AESOFF_MODE_ECB_ENC>(ybase, ybd, rk4, nr, src + row_off, dst + row_off, row_bytes, m == 0, iv, lane, kb);
+            else if (mode == AESOFF_MODE_ECB_DEC)
+                mode_blocks<NB, AESOFF_MODE_ECB_DEC>(ybase, ybd, rk4, nr, src + row_off, dst + row_off, row_bytes, m == 0, iv, lane, kb);
+            else
+                mode_blocks<NB, AESOFF_MODE_CBC_DEC>(ybase, ybd, rk4, nr, src + row_off, dst + row_off, row_bytes, m == 0, iv, lane, kb);
         }
     }
 }

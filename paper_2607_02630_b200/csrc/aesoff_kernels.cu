@@ -47,7 +47,8 @@ struct __align__(16) Slot {
     uint32_t ring_slot;     /* index of the request in dq / mailbox                             */
     uint32_t n_units;
     uint32_t n_rows;        /* rows of this chunk                                               */
-    uint32_t pad_[3];
+    uint32_t mode;          /* AESOFF_MODE_CTR / _ECB_ENC / _ECB_DEC / _CBC_DEC                 */
+    uint32_t pad_[2];
     uint32_t fine;          /* unit size: 0 rows (AESOFF_ROWS_PER_UNIT of them), AESOFF_FLAG_HALF half a row (128 blocks),
                                AESOFF_FLAG_FINE one k-iteration of a row (32 blocks)            */
 };                          /* 384 B */
@@ -62,7 +63,9 @@ struct __align__(16) CtaCtl {
     uint32_t stamp[AESOFF_SLOTS]; /* fill order, so that workers take the oldest open slot first */
     uint32_t busy[AESOFF_SLOTS];  /* 0 free, 1 filled and not yet completed                      */
     uint32_t exit_flag;
-    uint32_t pad[3];
+    uint32_t tables_ready;        /* set by a worker once the tables are filled: the service warp, which starts fetching
+                                     tickets while they are being built, needs them for a decrypting request's keys */
+    uint32_t pad[2];
     /* dispatcher CTAs: two landing areas for polls of the host ring (one is looked at while the next poll
      * flies): 32 descriptors as read from the ring, and a 33rd row for the control words that come with them */
     uint32_t stage[2][33][AESOFF_STAGE_STRIDE];
@@ -201,7 +204,30 @@ __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase,
         const CtrGeom g = ctr_geom(sl->desc.icb[0], sl->desc.icb[1], sl->desc.icb[2], sl->desc.icb[3]);
         const uint32_t n_units = sl->n_units;
         const uint32_t fine = sl->fine;
-        if (fine & AESOFF_FLAG_FINE) {
+        if (sl->mode != AESOFF_MODE_CTR) {
+            /* ECB / CBC-decrypt: the same units over rows of 256 blocks, no counter (the ICB words hold the IV) */
+            const uint4 iv = make_uint4(sl->desc.icb[0], sl->desc.icb[1], sl->desc.icb[2], sl->desc.icb[3]);
+            const uint32_t ybd = (ybase & ~0xffffu) + TD_OFF + (lane * 4u);
+            uint64_t m = sl->unit0_row;
+            uint32_t cnt = 1, kb0 = 0, kb1 = 8;
+            if (fine & AESOFF_FLAG_FINE) {
+                m += u >> 3;
+                kb0 = u & 7u;
+                kb1 = kb0 + 1u;
+            } else if (fine & AESOFF_FLAG_HALF) {
+                m += u >> 1;
+                kb0 = (u & 1u) * 4u;
+                kb1 = kb0 + 4u;
+            } else {
+                const uint32_t first = u * AESOFF_ROWS_PER_UNIT;
+                m += first;
+                cnt = sl->n_rows - first < AESOFF_ROWS_PER_UNIT ? sl->n_rows - first : AESOFF_ROWS_PER_UNIT;
+            }
+            if (kb1 - kb0 == 1u)
+                mode_request_rows<1>(sl->mode, ybase, ybd, rk4, nr, iv, src, dst, len, m, cnt, lane, kb0, kb1);
+            else
+                mode_request_rows<4>(sl->mode, ybase, ybd, rk4, nr, iv, src, dst, len, m, cnt, lane, kb0, kb1);
+        } else if (fine & AESOFF_FLAG_FINE) {
             const uint64_t m = (uint64_t)sl->unit0_row + (u >> 3);
             ctr_request_row<1>(ybase, rk4, nr, g, src, dst, len, m, lane, u & 7u, (u & 7u) + 1u);
         } else if (fine & AESOFF_FLAG_HALF) {
@@ -229,7 +255,7 @@ __device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase,
 /* ------------------------------------------------------------------------------------------ */
 /* Lane j < AESOFF_SLOTS owns slot j.  All lanes run in lock step; nothing here is on the
  * workers' critical path as long as at least one slot is open.                                 */
-__device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
+__device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase, uint32_t lane)
 {
     unsigned long long *g_ticket = reinterpret_cast<unsigned long long *>(P.counters + AESOFF_CNT_TICKET);
     const bool persistent = (P.mode == AESOFF_MODE_PERSISTENT);
@@ -374,6 +400,20 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
                 }
             }
             __syncwarp();
+            /* a decrypting request (ECB, CBC) runs the equivalent inverse cipher: its middle round keys go through
+             * InvMixColumns, here, once per chunk (60 words, two per lane; 0.3 % of a 4-row chunk's lookups) */
+            for (uint32_t m = ready_mask; m; m &= m - 1u) {
+                const uint32_t sj = __ffs(m) - 1;
+                Slot *sl = &c->slot[sj];
+                const uint32_t md = sl->desc.flags & 3u;
+                if (md == AESOFF_MODE_ECB_DEC || md == AESOFF_MODE_CBC_DEC) {
+                    while (lds_volatile(&c->tables_ready) == 0u) __nanosleep(100);
+                    uint32_t *rkw = reinterpret_cast<uint32_t *>(sl->rk4);
+                    const uint32_t nrr = sl->desc.nr, ybd = (ybase & ~0xffffu) + TD_OFF + (lane * 4u);
+                    for (uint32_t i = 4u + lane; i < 4u * nrr; i += 32u) rkw[i] = inv_mix_word(rkw[i], ybase, ybd);
+                }
+            }
+            __syncwarp();
             if (ready) {
                 Slot *sl = &c->slot[lane];
                 const unsigned long long rows = sl->desc.rows;
@@ -388,6 +428,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t lane)
                 sl->ring_slot = ring;
                 sl->n_units = n_units;
                 sl->fine = fine;
+                sl->mode = sl->desc.flags & 3u;
                 c->done[lane] = 0u;
                 c->stamp[lane] = stamp_base + __popc(ready_mask & ((1u << lane) - 1u));
                 c->busy[lane] = 1u;
@@ -616,7 +657,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         if (mine) {
             const unsigned long long len = ((unsigned long long)PW(AESOFF_PW_LEN + 1) << 32) | PW(AESOFF_PW_LEN);
             const unsigned long long nblocks = (len >> 4) + ((len & 15ull) ? 1ull : 0ull);
-            const uint32_t c0 = PW(AESOFF_PW_ICB + 3) >> 24;
+            const uint32_t c0 = (PW(AESOFF_PW_SPARE) & 3u) ? 0u : PW(AESOFF_PW_ICB + 3) >> 24; /* rows start at counter byte 0 */
             rows = nblocks ? (uint32_t)((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0u;
         }
         /* rows of this poll up to and including request k */
@@ -808,7 +849,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             d4[0] = make_uint4(PW(AESOFF_PW_ICB + 0), PW(AESOFF_PW_ICB + 1), PW(AESOFF_PW_ICB + 2), tg);
             d4[1] = make_uint4(PW(AESOFF_PW_ICB + 3), PW(AESOFF_PW_SRC), PW(AESOFF_PW_SRC + 1), tg);
             d4[2] = make_uint4(PW(AESOFF_PW_DST), PW(AESOFF_PW_DST + 1), PW(AESOFF_PW_LEN), tg);
-            d4[3] = make_uint4(PW(AESOFF_PW_LEN + 1), kw >> 24, fine, tg);
+            d4[3] = make_uint4(PW(AESOFF_PW_LEN + 1), kw >> 24, PW(AESOFF_PW_SPARE) & 3u, tg);
             d4[4] = make_uint4(nchunks, 1u << clog, (uint32_t)s, tg);
             d4[5] = make_uint4((uint32_t)(s >> 32), rows, 0u, tg);
             d4[6] = make_uint4((uint32_t)first_ticket, (uint32_t)(first_ticket >> 32), keyloc, tg);
@@ -887,7 +928,7 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
     const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(smem);
     /* tables on a 64 KiB boundary of the shared window so that PRMT can merge base and index */
     const uint32_t tbase = (sbase + 65535u) & ~65535u;
-    const uint32_t ctrl = (tbase - sbase >= CTRL_BYTES) ? sbase : tbase + TABLE_BYTES;
+    const uint32_t ctrl = (tbase - sbase >= CTRL_BYTES) ? sbase : tbase + TABLE_BYTES + TD_BYTES;
     CtaCtl *c = reinterpret_cast<CtaCtl *>(smem + (ctrl - sbase));
 
 #ifdef AESOFF_DEBUG
@@ -906,15 +947,17 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
         for (uint32_t i = lane; i < CTRL_BYTES / 4; i += 32u) reinterpret_cast<uint32_t *>(c)[i] = 0u;
         __threadfence_block();
         asm volatile("bar.arrive 1, %0;" ::"n"(AESOFF_CTA_THREADS) : "memory");
-        service_loop(P, c, lane);
+        service_loop(P, c, tbase | (lane * 4u), lane);
     } else if (warp == AESOFF_WORKER_WARPS + 1) {
         asm volatile("bar.sync 1, %0;" ::"n"(AESOFF_CTA_THREADS) : "memory");
         if (P.mode == AESOFF_MODE_PERSISTENT && blockIdx.x < P.n_disp) dispatcher_loop(P, c, tbase | (lane * 4u), lane, blockIdx.x);
     } else {
         if (tid == 0 && blockIdx.x == 0 && P.hctl) P.hctl[AESOFF_CTL_SMEMBASE] = sbase;
         fill_tables(tbase, P.T0, tid, AESOFF_WORKER_WARPS * 32u); /* worker threads only */
+        if (P.need_dec) fill_td(tbase, P.T0 + 256, tid, AESOFF_WORKER_WARPS * 32u);
         DBG_MAX(2); /* last CTA has its tables */
         asm volatile("bar.sync 1, %0;" ::"n"(AESOFF_CTA_THREADS) : "memory");
+        if (tid == 0) sts_volatile(&c->tables_ready, 1u);
         worker_loop(P, c, tbase | (lane * 4u), lane);
         DBG_MIN(6); /* first worker warp leaves */
         DBG_MAX(7); /* last worker warp leaves  */

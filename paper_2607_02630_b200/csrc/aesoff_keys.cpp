@@ -18,7 +18,7 @@
 namespace {
 
 uint8_t g_sbox[256];
-uint32_t g_T0[256];
+uint32_t g_T0[512]; /* T0, then Td0 (equivalent inverse cipher, FIPS-197 sec. 5.3.5) */
 std::once_flag g_once;
 
 inline uint8_t mul2(uint8_t a) { return (uint8_t)((a << 1) ^ ((a & 0x80) ? 0x1b : 0)); }
@@ -49,6 +49,14 @@ void build_tables()
         const uint8_t s = g_sbox[a], s2 = mul2(s), s3 = (uint8_t)(s2 ^ s);
         /* column (02,01,01,03)^T of MixColumns applied to S[a]; byte 0 of the word = row 0 */
         g_T0[a] = (uint32_t)s2 | ((uint32_t)s << 8) | ((uint32_t)s << 16) | ((uint32_t)s3 << 24);
+    }
+    /* Td0[x] = column (0e,09,0d,0b)^T of InvMixColumns (sec. 5.3.3) applied to InvSubBytes(x); products through the
+     * same logarithms.  The four bytes of an entry xor to InvSubBytes(x) itself (0e ^ 09 ^ 0d ^ 0b = 01), which is how
+     * the kernel's final round reads the inverse S-box out of this one table.                                       */
+    for (int a = 0; a < 256; ++a) {
+        const uint8_t x = g_sbox[a]; /* InvSubBytes(x) == a */
+        auto mul = [&](uint8_t c) -> uint32_t { return a ? alog[(lg[(uint8_t)a] + lg[c]) % 255] : 0u; };
+        g_T0[256 + x] = mul(0x0e) | (mul(0x09) << 8) | (mul(0x0d) << 16) | (mul(0x0b) << 24);
     }
 }
 

@@ -417,7 +417,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     ok = ok && cudaMalloc((void **)&e.counters, AESOFF_CNT_WORDS * 8) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.dev_done_seq, (size_t)e.R * 8) == cudaSuccess;
     ok = ok && cudaMalloc((void **)&e.dq_done, (size_t)e.R * 4) == cudaSuccess;
-    ok = ok && cudaMalloc((void **)&e.dT0, 256 * 4) == cudaSuccess;
+    ok = ok && cudaMalloc((void **)&e.dT0, 512 * 4) == cudaSuccess;
     if (!ok) {
         free_engine_memory(e);
         return fail(AES_E_NOMEM);
@@ -426,7 +426,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     memset(e.hmail, 0, (size_t)e.R * 8);
     ok = ok && cudaMemset(e.dev_done_seq, 0, (size_t)e.R * 8) == cudaSuccess;
     ok = ok && cudaMemset(e.dq, 0, (size_t)e.R * sizeof(aesoff_dq_entry_t)) == cudaSuccess; /* no tag matches yet */
-    ok = ok && cudaMemcpy(e.dT0, aesoff_T0_table(), 256 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+    ok = ok && cudaMemcpy(e.dT0, aesoff_T0_table(), 512 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
     if (ok) reset_key_ids(e);
     }
     /* sequence numbers never restart, so stale slot/mailbox values (< first_seq) can never match */
@@ -464,6 +464,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     p.fine_rows = o.fine_rows;
     p.first_seq = e.first_seq;
     p.n_disp = e.n_disp;
+    p.need_dec = 1;
     {   /* unit-size policy thresholds in rows (aesoff_shared.h AESOFF_TUNE_*); W = worker warps of the grid.
          * AESOFF_TUNE="a,b,c,d,e,f,g" overrides them (tuning experiments only). */
         const uint32_t W = (uint32_t)e.n_ctas * AESOFF_WORKER_WARPS;
@@ -645,14 +646,17 @@ extern "C" __attribute__((visibility("default"))) int aesoff_debug_dispatch_stat
 /* ============================================================================================ */
 /* submit / poll / wait (steps a2, a7)                                                          */
 /* ============================================================================================ */
-extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], const void *src, void *dst,
-                                       size_t len)
+namespace {
+/* mode: AESOFF_MODE_*; nonce: the ICB (CTR), the IV (CBC) or 16 zero bytes (ECB) */
+aes_handle_t submit_mode(aes_ctx_t *ctx, uint32_t mode, const uint8_t nonce[16], const void *src, void *dst, size_t len)
 {
     if (!ctx || !nonce) {
         fail(AES_E_INVAL);
         return 0;
     }
-    const int rc = check_buffers(src, dst, len);
+    int rc = check_buffers(src, dst, len);
+    if (rc == AES_OK && mode != AESOFF_MODE_CTR && (len & 15u)) rc = AES_E_INVAL;             /* whole blocks only */
+    if (rc == AES_OK && mode == AESOFF_MODE_CBC_DEC && len && src == dst) rc = AES_E_OVERLAP; /* see aesoff.h */
     if (rc != AES_OK) {
         fail(rc);
         return 0;
@@ -753,10 +757,25 @@ extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], 
     store_piece(w + 0, icb[0], icb[1], icb[2], tag);
     store_piece(w + 4, icb[3], (uint32_t)a_src, (uint32_t)(a_src >> 32), tag);
     store_piece(w + 8, (uint32_t)a_dst, (uint32_t)(a_dst >> 32), (uint32_t)a_len, tag);
-    store_piece(w + 12, (uint32_t)(a_len >> 32), kw, 0u, tag);
+    store_piece(w + 12, (uint32_t)(a_len >> 32), kw, mode, tag);
     /* later submits name ktab[id] once this request, which fills it, has completed */
     if (installing) __atomic_store_n(&ck.install_seq, s, __ATOMIC_RELEASE);
     return (aes_handle_t)(s | ((uint64_t)e.device << HANDLE_DEV_SHIFT));
+}
+const uint8_t k_zero_iv[16] = {0};
+} /* namespace */
+
+extern "C" aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16], const void *src, void *dst, size_t len)
+{
+    return submit_mode(ctx, AESOFF_MODE_CTR, nonce, src, dst, len);
+}
+extern "C" aes_handle_t aes_ecb_submit(aes_ctx_t *ctx, int decrypt, const void *src, void *dst, size_t len)
+{
+    return submit_mode(ctx, decrypt ? AESOFF_MODE_ECB_DEC : AESOFF_MODE_ECB_ENC, k_zero_iv, src, dst, len);
+}
+extern "C" aes_handle_t aes_cbc_decrypt_submit(aes_ctx_t *ctx, const uint8_t iv[16], const void *src, void *dst, size_t len)
+{
+    return submit_mode(ctx, AESOFF_MODE_CBC_DEC, iv, src, dst, len);
 }
 
 extern "C" int aes_poll(aes_handle_t h)
@@ -877,10 +896,24 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
                                     void *const *dsts, const size_t *lens, size_t n, int device, void *cuda_stream,
                                     uint32_t chunk_rows)
 {
+    return aes_mode_launch_batch(nullptr, ctxs, nonces, srcs, dsts, lens, n, device, cuda_stream, chunk_rows);
+}
+
+extern "C" int aes_mode_launch_batch(const int32_t *modes, aes_ctx_t *const *ctxs, const uint8_t *nonces,
+                                     const void *const *srcs, void *const *dsts, const size_t *lens, size_t n, int device,
+                                     void *cuda_stream, uint32_t chunk_rows)
+{
     if (n == 0) return AES_OK;
     if (!ctxs || !nonces || !srcs || !dsts || !lens) return fail(AES_E_INVAL);
     if (chunk_rows == 0) chunk_rows = 4;
-    if (chunk_rows > 64) return fail(AES_E_INVAL);
+    if (chunk_rows > 64 || !is_pow2(chunk_rows)) return fail(AES_E_INVAL);
+    bool need_dec = false;
+    for (size_t i = 0; modes && i < n; ++i) {
+        if (modes[i] < AES_MODE_CTR || modes[i] > AES_MODE_CBC_DEC) return fail(AES_E_INVAL);
+        if (modes[i] != AES_MODE_CTR && (lens[i] & 15u)) return fail(AES_E_INVAL);
+        if (modes[i] == AES_MODE_CBC_DEC && lens[i] && srcs[i] == dsts[i]) return fail(AES_E_OVERLAP);
+        need_dec = need_dec || modes[i] == AES_MODE_ECB_DEC || modes[i] == AES_MODE_CBC_DEC;
+    }
     if (device >= 0 && device < AESOFF_MAX_DEVICES && g_engs[device].running.load()) return fail(AES_E_BUSY);
     for (size_t i = 0; i < n; ++i) {
         if (!ctxs[i]) return fail(AES_E_INVAL);
@@ -905,7 +938,8 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     std::vector<uint32_t> crows(n), nch(n);
     uint64_t total = 0;
     for (size_t i = 0; i < n; ++i) {
-        request_geometry(lens[i], nonces[16 * i + 15], chunk_rows, 1u << 24, &rows[i], &crows[i], &nch[i]);
+        /* rows are aligned on counter byte 15 being 0 in CTR mode, on the start of the payload otherwise */
+        request_geometry(lens[i], (modes && modes[i]) ? 0 : nonces[16 * i + 15], chunk_rows, 1u << 24, &rows[i], &crows[i], &nch[i]);
         total += nch[i];
     }
     if (total >= (1ull << 30)) return fail(AES_E_INVAL);
@@ -936,9 +970,9 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         ok = ok && cudaMalloc((void **)&L.blob, L.blob_bytes) == cudaSuccess;
         ok = ok && cudaMalloc((void **)&L.dev_done_seq, L.cap_req * 8) == cudaSuccess;
         ok = ok && cudaMalloc((void **)&L.dq_done, L.cap_req * 4) == cudaSuccess;
-        ok = ok && cudaMalloc((void **)&L.dT0, 256 * 4) == cudaSuccess;
+        ok = ok && cudaMalloc((void **)&L.dT0, 512 * 4) == cudaSuccess;
         ok = ok && cudaHostAlloc((void **)&L.stage, L.blob_bytes, cudaHostAllocDefault) == cudaSuccess;
-        ok = ok && cudaMemcpy(L.dT0, aesoff_T0_table(), 256 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+        ok = ok && cudaMemcpy(L.dT0, aesoff_T0_table(), 512 * 4, cudaMemcpyHostToDevice) == cudaSuccess;
         ok = ok && cudaMemset(L.dq_done, 0, L.cap_req * 4) == cudaSuccess;
         ok = ok && cudaMemset(L.dev_done_seq, 0, L.cap_req * 8) == cudaSuccess;
         if (!ok) {
@@ -977,6 +1011,7 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
         d.dst = (uint64_t)(uintptr_t)dsts[i];
         d.len = (uint64_t)lens[i];
         d.nr = (uint32_t)ctxs[i]->nr;
+        d.flags = modes ? (uint32_t)modes[i] : AESOFF_MODE_CTR;
         d.nchunks = nch[i];
         d.chunk_rows = crows[i];
         d.seq = i + 1;
@@ -1047,6 +1082,7 @@ extern "C" int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonce
     p.TM = (uint32_t)L.cap_tickets;
     p.chunk_rows = chunk_rows;
     p.mode = AESOFF_MODE_DRAIN;
+    p.need_dec = need_dec ? 1u : 0u;
     p.first_seq = 1;
     uint64_t total_rows = 0;
     for (size_t i = 0; i < n; ++i) total_rows += rows[i];

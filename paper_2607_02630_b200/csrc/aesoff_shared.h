@@ -40,7 +40,13 @@
 #define AESOFF_KEY_BYTES       256u   /* one ktab entry: 60 round-key words + padding                     */
 #define AESOFF_KEY_IDS         4096u  /* ktab entries that installed contexts can own                      */
 #define AESOFF_KEY_NONE        0xffffu
-#define AESOFF_SMEM_BYTES      (200u * 1024u)
+#define AESOFF_SMEM_BYTES      (227u * 1024u) /* all of an SM: 4 encryption tables (128 KiB), Td0 (32 KiB), control block */
+
+/* what a request computes (descriptor word `flags`; SP 800-38A sec. 6.5, 6.1, 6.2) */
+#define AESOFF_MODE_CTR        0
+#define AESOFF_MODE_ECB_ENC    1
+#define AESOFF_MODE_ECB_DEC    2
+#define AESOFF_MODE_CBC_DEC    3
 
 #define AESOFF_MODE_PERSISTENT 0u
 #define AESOFF_MODE_DRAIN      1u
@@ -84,7 +90,7 @@
 #define AESOFF_PW_DST          6      /* 2 words */
 #define AESOFF_PW_LEN          8      /* 2 words */
 #define AESOFF_PW_KEY          10     /* key word, see AESOFF_KW_*                                  */
-#define AESOFF_PW_SPARE        11
+#define AESOFF_PW_SPARE        11     /* AESOFF_MODE_CTR / _ECB_ENC / _ECB_DEC / _CBC_DEC (the ICB words then hold the IV) */
 #define AESOFF_PW_RAWKEY       12     /* 8 words (second 64-byte line): the cipher key itself       */
 #define AESOFF_PW_WORDS        24
 #define AESOFF_PW_INDEX(p)     (((p) / 3) * 4 + (p) % 3)
@@ -158,7 +164,8 @@ typedef struct aesoff_params {
     uint64_t           *counters;
     uint32_t           *dq_done;
     uint64_t           *dev_done_seq;
-    const uint32_t     *T0;         /* 256 words: T0[x] = {02}S | S<<8 | S<<16 | {03}S<<24 */
+    const uint32_t     *T0;         /* 256 words: T0[x] = {02}S | S<<8 | S<<16 | {03}S<<24; then 256 words Td0 */
+    uint32_t            need_dec;   /* fill the Td0 table (always in persistent mode; drain: a decrypt request in the batch) */
     uint64_t            drain_total;
     uint32_t            R;          /* ring slots, power of two                          */
     uint32_t            TM;         /* ticket ring entries, power of two                 */
