@@ -614,6 +614,17 @@ def extra_cells(B, torch, dev, lds_peak, hbm_peak):
         for th in (1, 4):
             out["aes128_%s_w256_threads%d" % (name, th)] = cell(sz, 256, 150000, threads=th)
             out["aes128_%s_w1024_threads%d" % (name, th)] = cell(sz, 1024, 150000, threads=th)
+    # the other modes at the headline shape: 1 MiB requests, 64 in flight, out of place
+    nreq = 4000
+    nbuf = 128
+    icb = rng.integers(0, 256, size=(nreq, 16), dtype=np.uint8)
+    lens = np.full(nreq, MIB, dtype=np.uint64)
+    ps = np.asarray([base + (i % nbuf) * MIB for i in range(nreq)], dtype=np.uint64)
+    pd = np.asarray([base + (nbuf + i % nbuf) * MIB for i in range(nreq)], dtype=np.uint64)
+    for name, mode in (("ecb_encrypt", B.AES_MODE_ECB_ENC), ("ecb_decrypt", B.AES_MODE_ECB_DEC), ("cbc_decrypt", B.AES_MODE_CBC_DEC)):
+        B.aes_loop_run(icb[:128], ps[:128], pd[:128], lens[:128], window=64, ctx=ctx, want_latency=False, mode=mode)
+        r = B.aes_loop_run(icb, ps, pd, lens, window=64, ctx=ctx, want_latency=False, mode=mode)
+        out["aes128_%s_1MiB_w64" % name] = {"payload_gbs": r["bytes"] / r["elapsed_ns"], "frac_hbm_roof": 2 * r["bytes"] / r["elapsed_ns"] / hbm_peak}
     B.aes_ctx_destroy(ctx)
     return out
 

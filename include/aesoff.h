@@ -61,6 +61,12 @@ extern "C" {
 #define AES_E_BUSY      -9   /* call not allowed while the engine is running       */
 #define AES_E_NOMEM     -10  /* host or device allocation failed                   */
 
+/* what a request computes (SP 800-38A sec. 6.5, 6.1, 6.2) */
+#define AES_MODE_CTR     0
+#define AES_MODE_ECB_ENC 1
+#define AES_MODE_ECB_DEC 2
+#define AES_MODE_CBC_DEC 3
+
 typedef struct aes_ctx aes_ctx_t;     /* opaque; owns a copy of the expanded round keys */
 typedef uint64_t       aes_handle_t;  /* submission sequence number, from 1; 0 = invalid */
 
@@ -89,15 +95,21 @@ typedef struct aes_engine_opts {
     uint32_t n_dispatchers;   /* warps that poll the ring and cut requests into work items, one
                                  each on the first CTAs; consecutive batches of 32 sequence
                                  numbers go round them.  1..8; 0 = default 2               */
-    uint32_t reserved[2];     /* must be 0                                                */
+    uint32_t flags;           /* AES_ENGINE_* bits                                        */
+    uint32_t reserved[1];     /* must be 0                                                */
 } aes_engine_opts_t;
+/* Leave the decryption table out: aes_ecb_submit(decrypt) and aes_cbc_decrypt_submit then fail with AES_E_INVAL, and
+ * each persistent CTA takes 200 KiB of its SM's shared memory instead of 223 KiB, so that kernels of the process's own
+ * that need up to 27 KiB of shared memory per CTA can run beside the engine (with the table: up to 3 KiB).         */
+#define AES_ENGINE_NO_DECRYPT 1u
 
 /* Starts the engine on CUDA device `device`.  opts == NULL means all defaults.
  * Returns AES_OK, AES_E_BUSY if already running, AES_E_INVAL, AES_E_CUDA, AES_E_NOMEM.
  * While the engine runs, a device-wide synchronisation (cudaDeviceSynchronize,
  * cudaFree, torch.cuda.synchronize) blocks until aes_engine_stop(): synchronise
  * on streams or events instead.  Copies and other kernels run beside the engine
- * (it leaves 1,472 threads and 10 K registers per SM), with one catch: the FIRST
+ * (it leaves 1,472 threads, 10 K registers and a few KiB of shared memory per SM -- see AES_ENGINE_NO_DECRYPT --),
+ * with one catch: the FIRST
  * launch of a kernel whose module CUDA has not loaded yet (lazy loading) blocks
  * until the engine stops -- launch every kernel once before aes_engine_start, or
  * run with CUDA_MODULE_LOADING=EAGER.
@@ -248,10 +260,6 @@ int aes_ctr_launch_batch(aes_ctx_t *const *ctxs, const uint8_t *nonces,
 
 /* The same with a mode per request (modes == NULL: all CTR); nonces[16 i ..] is the ICB (CTR), the IV (CBC) or
  * ignored (ECB).  Restrictions of the modes as above.                                                              */
-#define AES_MODE_CTR     0
-#define AES_MODE_ECB_ENC 1
-#define AES_MODE_ECB_DEC 2
-#define AES_MODE_CBC_DEC 3
 int aes_mode_launch_batch(const int32_t *modes, aes_ctx_t *const *ctxs, const uint8_t *nonces,
                           const void *const *srcs, void *const *dsts,
                           const size_t *lens, size_t n,
@@ -282,6 +290,9 @@ typedef struct aes_loop_spec {
     const void *const  *srcs;
     void *const        *dsts;
     const size_t       *lens;
+    uint32_t            mode;       /* AES_MODE_CTR (0, the default), _ECB_ENC, _ECB_DEC, _CBC_DEC: what every request of
+                                       the run computes; nonces then hold the IVs (CBC) or are ignored (ECB)          */
+    uint32_t            reserved;   /* 0 */
 } aes_loop_spec_t;
 
 typedef struct aes_loop_result {

@@ -21,6 +21,7 @@ LIB_PATH = os.path.join(_PKG, "libaesoff.so")
 
 AES_OK = 0
 AES_FINE_ROWS_OFF = 0xFFFFFFFF
+AES_ENGINE_NO_DECRYPT = 1
 AES_E_INVAL = -1
 AES_E_KEYBITS = -2
 AES_E_ALIGN = -3
@@ -42,7 +43,7 @@ class AesOffError(RuntimeError):
 class aes_engine_opts_t(ctypes.Structure):
     _fields_ = [("ring_slots", ctypes.c_uint32), ("chunk_rows", ctypes.c_uint32), ("n_ctas", ctypes.c_uint32),
                 ("idle_exit_ms", ctypes.c_uint32), ("fine_rows", ctypes.c_uint32), ("n_dispatchers", ctypes.c_uint32),
-                ("reserved", ctypes.c_uint32 * 2)]
+                ("flags", ctypes.c_uint32), ("reserved", ctypes.c_uint32 * 1)]
 
 
 class aes_engine_info_t(ctypes.Structure):
@@ -65,7 +66,7 @@ class aes_loop_spec_t(ctypes.Structure):
     _fields_ = [("n", ctypes.c_size_t), ("window", ctypes.c_uint32), ("repeat", ctypes.c_uint32),
                 ("ctx", ctypes.c_void_p), ("keys", ctypes.c_void_p), ("keybits", ctypes.c_void_p),
                 ("nonces", ctypes.c_void_p), ("srcs", ctypes.c_void_p), ("dsts", ctypes.c_void_p),
-                ("lens", ctypes.c_void_p)]
+                ("lens", ctypes.c_void_p), ("mode", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
 
 
 class aes_loop_result_t(ctypes.Structure):
@@ -134,8 +135,8 @@ def _check(rc: int, where: str) -> None:
 
 # ---- engine ---------------------------------------------------------------------------------
 def aes_engine_start(device: int = 0, ring_slots: int = 0, chunk_rows: int = 0, n_ctas: int = 0,
-                     idle_exit_ms: int = 0, fine_rows: int = 0, n_dispatchers: int = 0) -> None:
-    o = aes_engine_opts_t(ring_slots, chunk_rows, n_ctas, idle_exit_ms, fine_rows, n_dispatchers)
+                     idle_exit_ms: int = 0, fine_rows: int = 0, n_dispatchers: int = 0, flags: int = 0) -> None:
+    o = aes_engine_opts_t(ring_slots, chunk_rows, n_ctas, idle_exit_ms, fine_rows, n_dispatchers, flags)
     _check(_lib.aes_engine_start(device, ctypes.byref(o)), "aes_engine_start")
 
 
@@ -268,7 +269,7 @@ def host_view(ptr: int, nbytes: int) -> np.ndarray:
 
 # ---- closed-loop executor ---------------------------------------------------------------------------
 def aes_loop_run(nonces, srcs, dsts, lens, window: int, ctx: int = 0, keys=None, keybits=None, repeat: int = 1,
-                 want_latency: bool = True, threads: int = 1) -> dict:
+                 want_latency: bool = True, threads: int = 1, mode: int = 0) -> dict:
     """Runs the native closed loop (see aes_loop_run in aesoff.h).  keys: n x 32 uint8 (16 used for
     128-bit keys) with keybits: n int32, or a shared ``ctx``.  Returns elapsed_ns, bytes, requests,
     ring_full_spins, max_in_flight and (optionally) lat_ns as a float64 array of n*repeat entries."""
@@ -279,6 +280,7 @@ def aes_loop_run(nonces, srcs, dsts, lens, window: int, ctx: int = 0, keys=None,
     spec = aes_loop_spec_t()
     spec.n, spec.window, spec.repeat = n, window, repeat
     spec.ctx = ctx or None
+    spec.mode = mode
     keep = []
     if keys is not None:
         a_keys = np.ascontiguousarray(np.asarray(keys, dtype=np.uint8)).reshape(-1)

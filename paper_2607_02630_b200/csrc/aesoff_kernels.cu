@@ -969,13 +969,10 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
 /* ------------------------------------------------------------------------------------------ */
 extern "C" int aesoff_launch_engine(const aesoff_params_t *params, int n_ctas, void *stream)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(aesoff_engine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)AESOFF_SMEM_BYTES);
-        if (e != cudaSuccess) return (int)e;
-        attr_set = true;
-    }
-    aesoff_engine_kernel<<<n_ctas, AESOFF_CTA_THREADS, AESOFF_SMEM_BYTES, (cudaStream_t)stream>>>(*params);
+    /* per device: the attribute belongs to the function as loaded on the current device */
+    cudaError_t e = cudaFuncSetAttribute(aesoff_engine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)AESOFF_SMEM_BYTES);
+    if (e != cudaSuccess) return (int)e;
+    const uint32_t smem = params->need_dec ? AESOFF_SMEM_BYTES : AESOFF_SMEM_BYTES_NODEC;
+    aesoff_engine_kernel<<<n_ctas, AESOFF_CTA_THREADS, smem, (cudaStream_t)stream>>>(*params);
     return (int)cudaGetLastError();
 }

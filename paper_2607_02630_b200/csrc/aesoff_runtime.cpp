@@ -83,6 +83,7 @@ struct Engine {
     int sm_count = 0;
     int n_ctas = 0;
     uint32_t n_disp = 1;
+    bool has_dec = true;                  /* the decryption table is in shared memory */
     uint32_t R = 0, Rm = 0, chunk_rows = 0, TM = 0;
     cudaStream_t stream = nullptr;
     aesoff_host_slot_t *hring = nullptr; /* pinned, mapped */
@@ -370,8 +371,7 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     aes_engine_opts_t o;
     memset(&o, 0, sizeof(o));
     if (opts) o = *opts;
-    for (int i = 0; i < 2; ++i)
-        if (o.reserved[i]) return fail(AES_E_INVAL);
+    if (o.reserved[0] || (o.flags & ~AES_ENGINE_NO_DECRYPT)) return fail(AES_E_INVAL);
     if (o.n_dispatchers == 0) o.n_dispatchers = AESOFF_DEF_DISPATCHERS;
     if (o.n_dispatchers > AESOFF_MAX_DISPATCHERS) return fail(AES_E_INVAL);
     if (o.ring_slots == 0) o.ring_slots = 2048;
@@ -464,7 +464,8 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     p.fine_rows = o.fine_rows;
     p.first_seq = e.first_seq;
     p.n_disp = e.n_disp;
-    p.need_dec = 1;
+    p.need_dec = (o.flags & AES_ENGINE_NO_DECRYPT) ? 0u : 1u;
+    e.has_dec = p.need_dec != 0;
     {   /* unit-size policy thresholds in rows (aesoff_shared.h AESOFF_TUNE_*); W = worker warps of the grid.
          * AESOFF_TUNE="a,b,c,d,e,f,g" overrides them (tuning experiments only). */
         const uint32_t W = (uint32_t)e.n_ctas * AESOFF_WORKER_WARPS;
@@ -592,7 +593,7 @@ extern "C" int aes_engine_info_device(int device, aes_engine_info_t *out)
     out->worker_warps_per_cta = AESOFF_WORKER_WARPS;
     out->ring_slots = e.R;
     out->chunk_rows = e.chunk_rows;
-    out->smem_bytes_per_cta = AESOFF_SMEM_BYTES;
+    out->smem_bytes_per_cta = e.has_dec ? AESOFF_SMEM_BYTES : AESOFF_SMEM_BYTES_NODEC;
     const uint64_t next = e.next_seq.load();
     out->submitted = next - 1;
     uint64_t pending = 0;
@@ -667,6 +668,10 @@ aes_handle_t submit_mode(aes_ctx_t *ctx, uint32_t mode, const uint8_t nonce[16],
         return 0;
     }
     Engine &e = *ep;
+    if ((mode == AESOFF_MODE_ECB_DEC || mode == AESOFF_MODE_CBC_DEC) && !e.has_dec) {
+        fail(AES_E_INVAL); /* started with AES_ENGINE_NO_DECRYPT */
+        return 0;
+    }
     aes_ctx_dev &ck = ctx->dev[e.device];
     /* counted BEFORE the running check: aes_engine_stop sets running = 2 and then waits for the count to
      * drop to 0, so a submit either fails here or has published its slot before the drain reads next_seq */
@@ -1144,7 +1149,7 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
     if (!spec || !res || !spec->nonces || !spec->srcs || !spec->dsts || !spec->lens) return fail(AES_E_INVAL);
     if (!spec->keys && !spec->ctx) return fail(AES_E_INVAL);
     if (spec->keys && !spec->keybits) return fail(AES_E_INVAL);
-    if (spec->n == 0 || spec->window == 0) return fail(AES_E_INVAL);
+    if (spec->n == 0 || spec->window == 0 || spec->mode > AES_MODE_CBC_DEC) return fail(AES_E_INVAL);
     const uint32_t running = g_running_mask.load(std::memory_order_acquire);
     if (!running) return fail(AES_E_STOPPED);
     uint32_t ring_total = 0; /* what can be in flight over all engines */
@@ -1183,7 +1188,7 @@ extern "C" int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res,
                 if (!ctx) return t_last_error;
             }
             const uint64_t ts = lat_ns ? ticks() : 0;
-            const aes_handle_t h = aes_ctr_submit(ctx, spec->nonces + 16 * i, spec->srcs[i], spec->dsts[i], spec->lens[i]);
+            const aes_handle_t h = submit_mode(ctx, spec->mode, spec->nonces + 16 * i, spec->srcs[i], spec->dsts[i], spec->lens[i]);
             if (spec->keys) aes_ctx_destroy(ctx);
             if (h == 0) {
                 if (t_last_error == AES_E_AGAIN) {

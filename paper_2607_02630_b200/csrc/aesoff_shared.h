@@ -40,7 +40,9 @@
 #define AESOFF_KEY_BYTES       256u   /* one ktab entry: 60 round-key words + padding                     */
 #define AESOFF_KEY_IDS         4096u  /* ktab entries that installed contexts can own                      */
 #define AESOFF_KEY_NONE        0xffffu
-#define AESOFF_SMEM_BYTES      (227u * 1024u) /* all of an SM: 4 encryption tables (128 KiB), Td0 (32 KiB), control block */
+#define AESOFF_SMEM_BYTES      (223u * 1024u) /* with the decryption table: control block, 4 encryption tables (128 KiB) on a
+                                                 64 KiB boundary of the shared window, Td0 (32 KiB); leaves 4 KiB of the SM */
+#define AESOFF_SMEM_BYTES_NODEC (200u * 1024u) /* without Td0: 27 KiB of the SM's shared memory stay free for other kernels */
 
 /* what a request computes (descriptor word `flags`; SP 800-38A sec. 6.5, 6.1, 6.2) */
 #define AESOFF_MODE_CTR        0

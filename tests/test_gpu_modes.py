@@ -149,3 +149,4 @@ def test_mode_errors(E):
         E.aes_cbc_decrypt_submit(ctx, bytes(16), t.data_ptr(), t.data_ptr() + 16, 1024)
     assert e.value.code == E.AES_E_OVERLAP
     E.aes_ctx_destroy(ctx)
+

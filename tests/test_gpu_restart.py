@@ -134,3 +134,43 @@ def test_other_kernels_run_beside_the_engine():
     finally:
         B.aes_engine_stop()
     B.aes_ctx_destroy(ctx)
+
+
+def test_engine_without_the_decryption_table():
+    """AES_ENGINE_NO_DECRYPT: 200 KiB of shared memory per CTA instead of 223; CTR and ECB-encrypt work, the
+    decrypting calls are refused."""
+    import gpu_util as G
+    import paper_2607_02630_b200.binding as B
+    from oracle import oracle as o
+
+    torch = G.torch_cuda()
+    torch.zeros(1, device="cuda:0")
+    torch.cuda.synchronize()
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 8500]))
+    key, iv = rng.bytes(24), rng.bytes(16)
+    data = np.frombuffer(rng.bytes(80000), dtype=np.uint8)
+    s, d = G.to_device(data), G.device_empty(len(data))
+    G.stream_sync()
+    ctx = B.aes_ctx_create(key)
+    B.aes_engine_start(0, idle_exit_ms=20000, flags=B.AES_ENGINE_NO_DECRYPT)
+    try:
+        assert B.aes_engine_info()["smem_bytes_per_cta"] == 200 * 1024
+        B.aes_wait(B.aes_ctr_submit(ctx, iv, s.data_ptr(), d.data_ptr(), len(data)))
+        assert d.cpu().numpy().tobytes() == o.ctr(key, iv, data)
+        B.aes_wait(B.aes_ecb_submit(ctx, False, s.data_ptr(), d.data_ptr(), len(data)))
+        assert d.cpu().numpy().tobytes() == o.ecb_encrypt(key, data)
+        for call in (lambda: B.aes_ecb_submit(ctx, True, s.data_ptr(), d.data_ptr(), len(data)),
+                     lambda: B.aes_cbc_decrypt_submit(ctx, iv, s.data_ptr(), d.data_ptr(), len(data))):
+            with pytest.raises(B.AesOffError) as e:
+                call()
+            assert e.value.code == B.AES_E_INVAL
+    finally:
+        B.aes_engine_stop()
+    B.aes_engine_start(0, idle_exit_ms=20000)
+    try:
+        assert B.aes_engine_info()["smem_bytes_per_cta"] == 223 * 1024
+        B.aes_wait(B.aes_cbc_decrypt_submit(ctx, iv, s.data_ptr(), d.data_ptr(), len(data)))
+        assert d.cpu().numpy().tobytes() == o.cbc_decrypt(key, iv, data)
+    finally:
+        B.aes_engine_stop()
+    B.aes_ctx_destroy(ctx)
