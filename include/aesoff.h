@@ -268,6 +268,14 @@ int aes_mode_launch_batch(const int32_t *modes, aes_ctx_t *const *ctxs, const ui
 /* ---- pinned host memory the GPU can address (for host-resident payloads) ----- */
 void *aes_host_alloc(size_t bytes);        /* NULL on error (AES_E_CUDA / AES_E_NOMEM) */
 void  aes_host_free(void *p);
+/* The same for memory the caller already owns -- the paper's request buffer is the server's own (j.buf,
+ * PAPER.md:132): page-locks [ptr, ptr + bytes) in place (cudaHostRegister, mapped and portable) so that it may be
+ * passed as src / dst of a submit at its own address (16-byte alignment of what is submitted still applies).
+ * Registration costs tens of microseconds per MiB: register a server's buffer pool once, not each request, and
+ * unregister only after the requests that use the range have completed.  AES_OK, AES_E_INVAL (NULL, zero bytes, already registered),
+ * AES_E_NOMEM, AES_E_CUDA.                                                                                      */
+int   aes_host_register(void *ptr, size_t bytes);
+int   aes_host_unregister(void *ptr);
 
 /* ---- closed-loop executor (the paper's worker pool) ----
  * Drives the running engine from native code so that a microsecond offload is not

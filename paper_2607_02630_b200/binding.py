@@ -102,6 +102,8 @@ def _load() -> ctypes.CDLL:
         "aes_ctr_launch_batch": (i32, [vp, vp, vp, vp, vp, sz, i32, vp, ctypes.c_uint32]),
         "aes_host_alloc": (vp, [sz]),
         "aes_host_free": (None, [vp]),
+        "aes_host_register": (i32, [vp, sz]),
+        "aes_host_unregister": (i32, [vp]),
         "aes_loop_run": (i32, [vp, vp, vp]),
         "aes_openloop_run": (i32, [vp, vp, i32, vp, vp]),
         "aes_loop_run_mt": (i32, [vp, ctypes.c_uint32, vp, vp]),
@@ -117,7 +119,7 @@ def _load() -> ctypes.CDLL:
 _lib = _load()
 EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_engine_info_device", "aes_engine_stop_device", "aes_route_flush", "aes_ctx_create", "aes_ctx_destroy",
            "aes_ctx_round_keys", "aes_ctr_submit", "aes_ecb_submit", "aes_cbc_decrypt_submit", "aes_mode_launch_batch", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
-           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_loop_run", "aes_loop_run_mt", "aes_openloop_run", "aes_calibrate")
+           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_host_register", "aes_host_unregister", "aes_loop_run", "aes_loop_run_mt", "aes_openloop_run", "aes_calibrate")
 
 
 def aes_strerror(code: int) -> str:
@@ -260,6 +262,15 @@ def aes_host_alloc(nbytes: int) -> int:
 
 def aes_host_free(ptr: int) -> None:
     _lib.aes_host_free(ptr)
+
+
+def aes_host_register(ptr: int, nbytes: int) -> None:
+    """Page-locks caller-owned host memory in place (e.g. ``ndarray.ctypes.data``) so that it can be submitted."""
+    _check(_lib.aes_host_register(ptr, nbytes), "aes_host_register")
+
+
+def aes_host_unregister(ptr: int) -> None:
+    _check(_lib.aes_host_unregister(ptr), "aes_host_unregister")
 
 
 def host_view(ptr: int, nbytes: int) -> np.ndarray:

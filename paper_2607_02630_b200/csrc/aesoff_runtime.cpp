@@ -862,6 +862,35 @@ extern "C" void aes_host_free(void *p)
     if (p) cudaFreeHost(p);
 }
 
+/* A buffer the server already owns (malloc, a slab, a network buffer: the paper's j.buf): page-lock it
+ * where it lies and make it GPU-addressable, so that it can be submitted as it is.                              */
+extern "C" int aes_host_register(void *ptr, size_t bytes)
+{
+    if (!ptr || bytes == 0) return fail(AES_E_INVAL);
+    const cudaError_t e = cudaHostRegister(ptr, bytes, cudaHostRegisterMapped | cudaHostRegisterPortable);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(e == cudaErrorMemoryAllocation ? AES_E_NOMEM : e == cudaErrorInvalidValue ? AES_E_INVAL : AES_E_CUDA);
+    }
+    void *dp = nullptr;
+    /* with unified addressing the device sees registered memory at its host address; the kernel uses that address */
+    if (cudaHostGetDevicePointer(&dp, ptr, 0) != cudaSuccess || dp != ptr) {
+        cudaGetLastError();
+        cudaHostUnregister(ptr);
+        return fail(AES_E_CUDA);
+    }
+    return AES_OK;
+}
+extern "C" int aes_host_unregister(void *ptr)
+{
+    if (!ptr) return fail(AES_E_INVAL);
+    if (cudaHostUnregister(ptr) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(AES_E_INVAL);
+    }
+    return AES_OK;
+}
+
 /* ============================================================================================ */
 /* launch backend: the paper's mechanism (own stream + event)                      */
 /* ============================================================================================ */

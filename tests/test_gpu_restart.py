@@ -174,3 +174,41 @@ def test_engine_without_the_decryption_table():
     finally:
         B.aes_engine_stop()
     B.aes_ctx_destroy(ctx)
+
+
+def test_ordinary_host_memory_after_registration():
+    """The paper's buffer is the server's own memory (j.buf): a numpy array from the ordinary heap is
+    page-locked in place with aes_host_register and submitted at its own address, in place and out of place."""
+    import gpu_util as G
+    import paper_2607_02630_b200.binding as B
+    from oracle import oracle as o
+
+    torch = G.torch_cuda()
+    torch.zeros(1, device="cuda:0")
+    torch.cuda.synchronize()
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 8600]))
+    n = (1 << 20) + 4096 + 7
+    pool = np.zeros(3 * (1 << 21), dtype=np.uint8)             # the "server's" buffer pool, registered once
+    base = (pool.ctypes.data + 63) & ~63
+    B.aes_host_register(pool.ctypes.data, pool.nbytes)
+    with pytest.raises(B.AesOffError):
+        B.aes_host_register(pool.ctypes.data, pool.nbytes)      # twice is an error, not a crash
+    off = base - pool.ctypes.data
+    src, dst = pool[off:off + n], pool[off + (1 << 21):off + (1 << 21) + n]
+    src[:] = np.frombuffer(rng.bytes(n), dtype=np.uint8)
+    plain = src.copy()
+    key, icb = rng.bytes(32), rng.bytes(16)
+    ctx = B.aes_ctx_create(key)
+    B.aes_engine_start(0, idle_exit_ms=20000)
+    try:
+        B.aes_wait(B.aes_ctr_submit(ctx, icb, src.ctypes.data, dst.ctypes.data, n))
+        assert dst.tobytes() == o.ctr(key, icb, plain)
+        B.aes_wait(B.aes_ctr_submit(ctx, icb, src.ctypes.data, src.ctypes.data, n))   # in place, as accel_encrypt(j.buf, j.len)
+        assert src.tobytes() == o.ctr(key, icb, plain)
+        dev = G.device_empty(n)                                                      # host -> device as well
+        B.aes_wait(B.aes_ctr_submit(ctx, icb, src.ctypes.data, dev.data_ptr(), n))
+        assert dev.cpu().numpy()[:n].tobytes() == plain.tobytes()
+    finally:
+        B.aes_engine_stop()
+    B.aes_host_unregister(pool.ctypes.data)
+    B.aes_ctx_destroy(ctx)
