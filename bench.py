@@ -915,6 +915,13 @@ def extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, s
         cal = B.aes_calibrate(local_rank)
         cal["lookup_pipe_frac_of_nominal"] = cal["lookups_per_clk_per_sm"] / 32.0
         cal["main_round_frac_of_nominal"] = cal["round_lookups_per_clk_per_sm"] / 32.0
+        # the bitsliced alternative: one warp-wide S-box evaluation covers 32 lanes x 32 bytes; an AES-128
+        # block needs 160 byte substitutions; MixColumns, AddRoundKey and the bit transposes come on top and are NOT counted
+        cal["bitslice_subbytes_only_aes128_gbs"] = (cal["bitslice_sboxes_per_clk_per_sm"] * 1024.0 * cal["sm_count"] *
+                                                    cal["sm_mhz"] * 1e6 / 160.0 * 16.0 / 1e9)
+        cal["bitslice_how"] = ("tower-field circuit generated and checked by csrc/gen_bitslice_sbox.py, 117 LOP3 per S-box in the SASS, "
+                               "verified on all 256 inputs on the GPU (bitslice_mismatches must be 0), 4 independent chains per thread; "
+                               "the figure is the ceiling of SubBytes ALONE for a bitsliced AES-128")
         cal["how"] = ("aes_calibrate: microkernels with the engine's table layout and launch shape; nominal = 32 lookups and "
                       "2 warp-wide ALU instructions per clock per SM (guides/B300_MICROARCH.md)")
         res["calibration"] = cal

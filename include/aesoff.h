@@ -321,7 +321,7 @@ int aes_loop_run(const aes_loop_spec_t *spec, aes_loop_result_t *res, double *la
 int aes_loop_run_mt(const aes_loop_spec_t *spec, uint32_t nthreads, aes_loop_result_t *res, double *lat_ns);
 
 /* ---- calibration ---------------------------
- * Runs three microkernels with the engine's own table layout and launch shape and reports what the
+ * Runs microkernels with the engine's own table layout and launch shape and reports what the
  * units the cipher leans on deliver on this GPU: table lookups (PRMT + conflict-free LDS.32) per
  * clock per SM, warp-wide ALU instructions (PRMT / LOP3) per clock per SM, the lookup rate of the
  * cipher's main round as it stands, and the GB/s (read + write) of 128-bit L2-only loads and
@@ -337,6 +337,10 @@ typedef struct aes_calib {
     double  round_lookups_per_clk_per_sm; /* lookups per clock per SM of the cipher's own main
                                              round (4 PRMT + 4 LDS + 2 LOP3 per column): what the
                                              two pipes deliver together                        */
+    double  bitslice_sboxes_per_clk_per_sm; /* the alternative to tables: warp-wide evaluations of a bitsliced
+                                             S-box (32 lanes x 32 bytes each) per clock per SM  */
+    int32_t bitslice_mismatches;         /* of that circuit against S[x] over all 256 inputs: must be 0  */
+    int32_t reserved2;
 } aes_calib_t;
 int aes_calibrate(int device, aes_calib_t *out);
 

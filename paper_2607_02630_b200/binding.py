@@ -59,7 +59,9 @@ class aes_engine_info_t(ctypes.Structure):
 class aes_calib_t(ctypes.Structure):
     _fields_ = [("lookups_per_clk_per_sm", ctypes.c_double), ("alu_instr_per_clk_per_sm", ctypes.c_double),
                 ("copy_gbs", ctypes.c_double), ("sm_mhz", ctypes.c_double), ("sm_count", ctypes.c_int32),
-                ("reserved", ctypes.c_int32), ("round_lookups_per_clk_per_sm", ctypes.c_double)]
+                ("reserved", ctypes.c_int32), ("round_lookups_per_clk_per_sm", ctypes.c_double),
+                ("bitslice_sboxes_per_clk_per_sm", ctypes.c_double), ("bitslice_mismatches", ctypes.c_int32),
+                ("reserved2", ctypes.c_int32)]
 
 
 class aes_loop_spec_t(ctypes.Structure):
@@ -338,4 +340,4 @@ def aes_calibrate(device: int = 0) -> dict:
     """Calibration microkernels (see aes_calibrate in aesoff.h)."""
     c = aes_calib_t()
     _check(_lib.aes_calibrate(device, ctypes.byref(c)), "aes_calibrate")
-    return {k: getattr(c, k) for k, _ in aes_calib_t._fields_ if k != "reserved"}
+    return {k: getattr(c, k) for k, _ in aes_calib_t._fields_ if not k.startswith("reserved")}

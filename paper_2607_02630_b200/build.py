@@ -18,7 +18,7 @@ _ROOT = os.path.dirname(_PKG)
 CSRC = os.path.join(_PKG, "csrc")
 SO = os.path.join(_PKG, "libaesoff.so")
 SOURCES = ["aesoff_kernels.cu", "aesoff_calib.cu", "aesoff_runtime.cpp", "aesoff_keys.cpp", "aesoff_router.cpp"]
-HEADERS = ["aesoff_shared.h", "aesoff_internal.h", "aesoff_cipher.cuh", os.path.join(_ROOT, "include", "aesoff.h")]
+HEADERS = ["aesoff_shared.h", "aesoff_internal.h", "aesoff_cipher.cuh", "aesoff_bitslice.cuh", os.path.join(_ROOT, "include", "aesoff.h")]
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-lineinfo",

@@ -9,12 +9,17 @@
  *   round    the cipher's main round as it stands (per column 4 PRMT + 4 LDS + 2 LOP3, 4 blocks per lane):
  *            what the two pipes deliver together, i.e. the ceiling of the kernel's inner loop.
  *   copy     128-bit L2-only loads and stores of a buffer larger than L2: the payload path's HBM rate.
+ *   bitslice the alternative the table form was chosen against: a bitsliced S-box
+ *            (aesoff_bitslice.cuh: tower-field circuit derived and checked by gen_bitslice_sbox.py), first
+ *            verified on all 256 inputs against S[x] as read out of T0, then run as 4 independent chains
+ *            per thread: S-box evaluations (32 lanes x 32 bytes each) per clock per SM.
  *
  * Nothing here is on the product path; aes_calibrate() is called by bench.py and the tests only.
  */
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include "aesoff_bitslice.cuh"
 #include "aesoff_cipher.cuh"
 #include "aesoff_internal.h"
 
@@ -84,6 +89,50 @@ calib_lookup_kernel(const uint32_t *T0, uint32_t iters, uint32_t *sink, unsigned
     }
 }
 
+constexpr int BS_CHAINS = 4;
+__global__ void __launch_bounds__(CALIB_THREADS, 1)
+calib_bitslice_kernel(const uint32_t *T0, uint32_t iters, uint32_t *sink, unsigned long long *cycles, uint32_t *mismatches)
+{
+    /* correctness first: pass p covers the byte values 32 p + j, j = lane-independent bit position */
+    if (blockIdx.x == 0 && threadIdx.x < 8) {
+        const uint32_t p = threadIdx.x;
+        uint32_t x[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            x[k] = 0;
+            for (uint32_t j = 0; j < 32; ++j) x[k] |= (((32u * p + j) >> k) & 1u) << j;
+        }
+        bitslice_sbox(x);
+        uint32_t bad = 0;
+        for (uint32_t j = 0; j < 32; ++j) {
+            uint32_t s = 0;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) s |= ((x[k] >> j) & 1u) << k;
+            if (s != ((__ldg(T0 + 32u * p + j) >> 8) & 0xffu)) ++bad; /* byte 1 of T0[v] is S[v] */
+        }
+        if (bad) atomicAdd(mismatches, bad);
+    }
+    uint32_t st[BS_CHAINS][8];
+#pragma unroll
+    for (int c = 0; c < BS_CHAINS; ++c)
+#pragma unroll
+        for (int k = 0; k < 8; ++k) st[c][k] = (threadIdx.x * 2654435761u) ^ ((c * 8 + k) * 0x9e3779b9u) ^ blockIdx.x;
+    __syncthreads();
+    const long long t0 = clock64();
+    for (uint32_t it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int c = 0; c < BS_CHAINS; ++c) bitslice_sbox(st[c]);
+    }
+    const long long t1 = clock64();
+    uint32_t acc = 0;
+#pragma unroll
+    for (int c = 0; c < BS_CHAINS; ++c)
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc ^= st[c][k];
+    if (acc == 0x12345678u) sink[0] = acc;
+    if (threadIdx.x == 0) cycles[blockIdx.x] = (unsigned long long)(t1 - t0);
+}
+
 __global__ void __launch_bounds__(CALIB_THREADS, 2) calib_copy_kernel(const uint4 *src, uint4 *dst, size_t n16)
 {
     const size_t stride = (size_t)gridDim.x * blockDim.x;
@@ -95,7 +144,7 @@ __global__ void __launch_bounds__(CALIB_THREADS, 2) calib_copy_kernel(const uint
 /* Fills out[0..5]: lookups per clock per SM, ALU instructions (warp-wide) per clock per SM, copy GB/s
  * (read + write bytes), SM clock in MHz during the lookup run, SM count, lookups per clock per SM of the
  * cipher's own main-round instruction mix.  Returns 0 or a CUDA error.                                   */
-extern "C" int aesoff_run_calibration(int device, double out[6])
+extern "C" int aesoff_run_calibration(int device, double out[8])
 {
     cudaError_t e = cudaSetDevice(device);
     if (e != cudaSuccess) return (int)e;
@@ -132,6 +181,24 @@ extern "C" int aesoff_run_calibration(int device, double out[6])
         /* in-kernel cycles over in-kernel globaltimer nanoseconds (an event time would include launch and table fill) */
         if (with_loads == 1 && ns0) mhz = (double)c0 * 1e3 / (double)ns0;
     }
+    /* bitsliced S-box: verified, then timed */
+    double bs_rate = 0, bs_bad = -1;
+    {
+        uint32_t *mm = nullptr;
+        if (ok && cudaMalloc(&mm, 4) == cudaSuccess) {
+            const uint32_t bs_iters = 2048;
+            cudaMemset(mm, 0, 4);
+            calib_bitslice_kernel<<<sms, CALIB_THREADS>>>(dT0, 16, sink, cyc, mm);
+            calib_bitslice_kernel<<<sms, CALIB_THREADS>>>(dT0, bs_iters, sink, cyc, mm);
+            unsigned long long c0 = 0;
+            uint32_t bad = 0;
+            ok = cudaDeviceSynchronize() == cudaSuccess && cudaMemcpy(&c0, cyc, sizeof(c0), cudaMemcpyDeviceToHost) == cudaSuccess &&
+                 cudaMemcpy(&bad, mm, 4, cudaMemcpyDeviceToHost) == cudaSuccess;
+            if (ok && c0) bs_rate = (double)(CALIB_THREADS / 32) * bs_iters * BS_CHAINS / (double)c0;
+            bs_bad = (double)bad;
+            cudaFree(mm);
+        }
+    }
     /* copy: 2 x 1 GiB, three passes, best */
     double copy_gbs = 0;
     uint4 *a = nullptr, *b = nullptr;
@@ -166,5 +233,7 @@ extern "C" int aesoff_run_calibration(int device, double out[6])
     out[3] = mhz;
     out[4] = (double)sms;
     out[5] = res[2];
+    out[6] = bs_rate;
+    out[7] = bs_bad;
     return 0;
 }

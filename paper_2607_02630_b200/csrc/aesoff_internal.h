@@ -50,6 +50,6 @@ const uint32_t *aesoff_T0_table();
 int aesoff_key_expand(const uint8_t *key, int keybits, uint32_t rk[60]);
 
 extern "C" int aesoff_launch_engine(const aesoff_params_t *params, int n_ctas, void *stream);
-extern "C" int aesoff_run_calibration(int device, double out[6]);
+extern "C" int aesoff_run_calibration(int device, double out[8]);
 
 #endif

@@ -1266,7 +1266,7 @@ extern "C" int aes_calibrate(int device, aes_calib_t *out)
     if (device >= 0 && device < AESOFF_MAX_DEVICES && g_engs[device].running.load()) return fail(AES_E_BUSY);
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(AES_E_CUDA);
-    double v[6];
+    double v[8];
     if (aesoff_run_calibration(device, v) != 0) return fail(AES_E_CUDA);
     out->lookups_per_clk_per_sm = v[0] * 32.0; /* the kernel counts warp-wide LDS instructions */
     out->alu_instr_per_clk_per_sm = v[1];
@@ -1275,6 +1275,9 @@ extern "C" int aes_calibrate(int device, aes_calib_t *out)
     out->sm_count = (int32_t)v[4];
     out->reserved = 0;
     out->round_lookups_per_clk_per_sm = v[5] * 32.0;
+    out->bitslice_sboxes_per_clk_per_sm = v[6];
+    out->bitslice_mismatches = (int32_t)v[7];
+    out->reserved2 = 0;
     return AES_OK;
 }
 

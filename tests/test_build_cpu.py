@@ -57,3 +57,13 @@ def test_sass_has_the_instructions_the_design_rests_on(cubin):
     assert re.search(r"LDG\.E\.128\.STRONG\.GPU", sass) and re.search(r"STG\.E\.128\.STRONG\.GPU", sass)  # L2-only 128-bit payload
     assert "MEMBAR.SC.SYS" in sass or "MEMBAR.ALL.SYS" in sass or "ERRBAR" in sass  # system-scope fence before the mailbox
     assert re.search(r"BAR\.ARV|BAR\.SYNC", sass)                    # the named barriers of the start-up overlap
+
+
+def test_bitslice_circuit_is_what_the_generator_derives():
+    """aesoff_bitslice.cuh is generated: the committed file must be exactly what gen_bitslice_sbox.py prints (the
+    generator checks its derivation against the S-box definition for all 256 inputs before it prints anything)."""
+    import sys
+
+    gen = os.path.join(CSRC, "gen_bitslice_sbox.py")
+    p = subprocess.run([sys.executable, gen], stdout=subprocess.PIPE, text=True, check=True)
+    assert p.stdout == open(os.path.join(CSRC, "aesoff_bitslice.cuh")).read()

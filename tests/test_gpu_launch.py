@@ -173,6 +173,10 @@ def test_calibration_microkernels(P):
     assert 26.0 <= c["round_lookups_per_clk_per_sm"] <= 32.5, c
     assert 1.7 <= c["alu_instr_per_clk_per_sm"] <= 2.1, c
     assert c["copy_gbs"] > 3000.0, c
+    # the bitsliced S-box the table form was chosen against: the generated circuit is right on all 256 inputs, and at
+    # 117 LOP3 per evaluation it cannot run faster than the ALU pipe allows (2 warp-wide instructions per clock per SM)
+    assert c["bitslice_mismatches"] == 0, c
+    assert 0.005 <= c["bitslice_sboxes_per_clk_per_sm"] <= 2.1 / 117.0 * 1.05, c
 
 
 @pytest.mark.parametrize("low4", ["01fffe00", "01ffff00", "ffffff37", "ffffffff", "00000000", "a1b2ff9c"])
