@@ -35,7 +35,8 @@ using namespace aesoff;
 
 namespace {
 
-constexpr uint32_t AESOFF_STAGE_STRIDE = 36; /* words per staged descriptor: 32 + padding against bank conflicts */
+constexpr uint32_t AESOFF_STAGE_STRIDE = 36;
+constexpr uint32_t AESOFF_LANDINGS = 4;      /* landing areas for polls of the host ring: up to three in flight + the one looked at */ /* words per staged descriptor: 32 + padding against bank conflicts */
 
 /* ------------------------------------------------------------------------------------------ */
 /* per-CTA control block in shared memory                                                      */
@@ -63,12 +64,13 @@ struct __align__(16) CtaCtl {
     uint32_t stamp[AESOFF_SLOTS]; /* fill order, so that workers take the oldest open slot first */
     uint32_t busy[AESOFF_SLOTS];  /* 0 free, 1 filled and not yet completed                      */
     uint32_t exit_flag;
+    uint32_t disp_stat[4];        /* dispatcher: requests cut into 1/8 rows / half rows / rows so far, and "changed" */
     uint32_t tables_ready;        /* set by a worker once the tables are filled: the service warp, which starts fetching
                                      tickets while they are being built, needs them for a decrypting request's keys */
     uint32_t pad[2];
-    /* dispatcher CTAs: two landing areas for polls of the host ring (one is looked at while the next poll
-     * flies): 32 descriptors as read from the ring, and a 33rd row for the control words that come with them */
-    uint32_t stage[2][33][AESOFF_STAGE_STRIDE];
+    /* dispatcher CTAs: landing areas for polls of the host ring (one is looked at while the next ones fly):
+     * 32 descriptors as read from the ring, and a 33rd row for the control words that come with them */
+    uint32_t stage[AESOFF_LANDINGS][33][AESOFF_STAGE_STRIDE];
 };
 constexpr uint32_t CTRL_BYTES = sizeof(CtaCtl);
 constexpr uint32_t CLAIM_EXIT = 0xffffffffu;
@@ -112,7 +114,16 @@ __device__ __forceinline__ void cp_async16(void *smem_dst, const void *gsrc)
                  : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+/* waits until at most `pending` of this thread's newest copy groups are still in flight (groups complete in order) */
+__device__ __forceinline__ void cp_async_wait_but(uint32_t pending)
+{
+    if (pending == 0u)
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+    else if (pending == 1u)
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+    else
+        asm volatile("cp.async.wait_group 2;" ::: "memory");
+}
 __device__ __forceinline__ unsigned long long globaltimer_ns()
 {
     unsigned long long t;
@@ -481,10 +492,8 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
     unsigned long long my_pub = 0;             /* chain.published while I hold the token       */
     unsigned long long oldest = P.first_seq;   /* every seq below this is known to be complete */
     unsigned long long base = 0;               /* first ticket of request `oldest` at the last scan */
-    unsigned long long last_activity = globaltimer_ns(), seen_next = 0;
+    uint32_t last_activity_us = (uint32_t)(globaltimer_ns() >> 10), seen_next = 0; /* dispatcher 0's idle timer (1.024 us units) */
     uint32_t wide = 0;                         /* 0: poll 8 slots, 1: poll 32                  */
-    uint32_t n_eighths = 0, n_halves = 0, n_rows = 0;
-    bool stats_dirty = false;
 #ifdef AESOFF_DISP_STATS
     uint32_t dbg_takes = 0, dbg_reqs = 0, dbg_empty = 0;
     unsigned long long dbg_wait = 0, dbg_work = 0;
@@ -499,14 +508,15 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
      * processed: the PCIe round trip of the next one runs under the on-chip work of this one.  (The polls used to
      * live in 32 registers; whenever ptxas let an LDS of the processing code share a scoreboard with them, that
      * LDS waited out the PCIe round trip: +1.6 us on every request, found with a time stamp.)                */
-    uint32_t cur = 0; /* landing area being looked at */
+    uint32_t cur = 0;                      /* landing area being looked at */
+    uint32_t n_issued = 0, n_looked = 0;   /* polls issued / looked at: area of poll i is i % AESOFF_LANDINGS */
 #define AUX_CTL   0   /* row 32 of a landing area: words 0..3 host control words (0 = stop) */
 #define AUX_CHAIN 4   /*   4..7   the token                                                  */
 #define AUX_TKT   8   /*   8..11  {tickets reserved, tickets published}                      */
 #define AUX_IDLE  12  /*   12..15 {idle CTAs, quit, long queue}                              */
 #define ISSUE_POLL(bseq, q, ring)                                                                            \
     do {                                                                                                     \
-        uint32_t(*land_)[AESOFF_STAGE_STRIDE] = c->stage[cur ^ 1u];                                          \
+        uint32_t(*land_)[AESOFF_STAGE_STRIDE] = c->stage[n_issued++ % AESOFF_LANDINGS];                      \
         const uint32_t nload_ = !(ring) ? 0u : wide ? 8u : 2u;                                               \
         const uint32_t q_ = wide ? 0u : (q);                                                                 \
         _Pragma("unroll") for (uint32_t j = 0; j < 8; ++j)                                                  \
@@ -527,7 +537,6 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         }                                                                                                    \
         cp_async_commit();                                                                                   \
     } while (0)
-    bool repoll = true; /* no poll in flight for (b_seq, pos) */
     /* Only the dispatcher that holds the token can take requests now; what the others read is a prefetch.  Polls
      * of several warps queue up behind one another on PCIe (four of them polling flat out added 4 us to a lone
      * request), so: the holder polls continuously; the others only watch the token -- unless the holder has
@@ -535,18 +544,26 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
      * the dispatchers whose batch comes next or next but one read their slots ahead of the token.            */
     unsigned long long token_at = (K == 1u) ? b_seq : 0ull; /* chain.next as last seen */
     bool queue_long = false;     /* the holder's last word on it */
+    uint32_t empties = 0;        /* looks in a row that found nothing */
 
     for (;;) {
         /* ---- phase 1: the PCIe round trip ---------------------------------------------------- */
-        if (repoll) {
+        {
             const bool holder = have_token || token_at == b_seq + pos;
             const bool near = holder || (queue_long && token_at + 2ull * AESOFF_BATCH >= b_seq);
-            if (!holder) __nanosleep(queue_long ? 400u : 3000u); /* device words only: no PCIe read (ISSUE_POLL) */
-            ISSUE_POLL(b_seq, pos, near);
+            /* The holder of the token, once it has found the ring empty (an idle engine: the latency case), keeps `depth` polls in flight, each issued when an older one has been looked at: a request
+             * that arrives waits a fraction of a PCIe round trip for the next poll to leave instead of half of one
+             * (lone 4 KiB 8.9 -> 8.25 us with three; 3 KiB per microsecond of PCIe reads).  Polls that were issued before
+             * a request was taken would show it again: they are skipped, not looked at (see the end of the loop).   */
+            const uint32_t depth = (holder && empties >= 1u) ? P.tune[AESOFF_TUNE_POLL_DEPTH] : 1u;
+            if (!holder && n_issued == n_looked) __nanosleep(queue_long ? 400u : 3000u); /* device words only: no PCIe read (ISSUE_POLL) */
+            while (n_issued - n_looked < depth) {
+                if (n_issued != n_looked) __nanosleep(P.tune[AESOFF_TUNE_POLL_GAP]); /* spread them over a round trip */
+                ISSUE_POLL(b_seq, pos, near);
+            }
         }
-        repoll = false;
-        cp_async_wait_all();
-        cur ^= 1u;
+        cp_async_wait_but(n_issued - n_looked - 1u);
+        cur = n_looked++ % AESOFF_LANDINGS;
         __syncwarp();
 #ifdef AESOFF_DISP_STATS
         const unsigned long long dbg_t0 = globaltimer_ns(); /* the poll has landed */
@@ -582,8 +599,8 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                 ISSUE_POLL(b_seq, pos + n, true);
         }
 #endif
+        empties = n ? 0u : empties + 1u;
         if (n == 0) {
-            repoll = true;
             if (queue_long && (have_token || chain_next == b_seq + pos)) { /* the queue has run dry: the others stop reading ahead */
                 queue_long = false;
                 if (lane == 0) *(reinterpret_cast<volatile uint32_t *>(g_quit) + 1) = 0u;
@@ -591,13 +608,14 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
 #ifdef AESOFF_DISP_STATS
             ++dbg_empty;
 #endif
-            if (stats_dirty) {
+            if (c->disp_stat[3]) {
                 /* not on a request's way: a PCIe write in flight would hold up the next fence */
                 if (lane == 0) {
                     volatile uint32_t *st = P.hctl + AESOFF_CTL_STATS + AESOFF_CTL_STAT_WORDS * d;
-                    st[AESOFF_CTL_CUT_EIGHTHS] = n_eighths;
-                    st[AESOFF_CTL_CUT_HALVES] = n_halves;
-                    st[AESOFF_CTL_CUT_ROWS] = n_rows;
+                    st[AESOFF_CTL_CUT_EIGHTHS] = c->disp_stat[0];
+                    st[AESOFF_CTL_CUT_HALVES] = c->disp_stat[1];
+                    st[AESOFF_CTL_CUT_ROWS] = c->disp_stat[2];
+                    c->disp_stat[3] = 0u;
 #ifdef AESOFF_DISP_STATS
                     st[AESOFF_CTL_DBG_TAKES] = dbg_takes;
                     st[AESOFF_CTL_DBG_REQS] = dbg_reqs;
@@ -606,17 +624,17 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                     st[AESOFF_CTL_DBG_EMPTY] = dbg_empty;
 #endif
                 }
-                stats_dirty = false;
+                __syncwarp();
             }
             bool quit = stop != 0 || quit_word != 0;
             if (!quit && d == 0 && P.idle_exit_ms) {
                 /* the idle timer is dispatcher 0's: it runs while no dispatcher takes anything, and fires only
                  * when everything that was accepted has completed */
-                const unsigned long long now = globaltimer_ns();
-                if (chain_next != seen_next) {
-                    seen_next = chain_next;
-                    last_activity = now;
-                } else if (now - last_activity > (unsigned long long)P.idle_exit_ms * 1000000ull) {
+                const uint32_t now = (uint32_t)(globaltimer_ns() >> 10);
+                if ((uint32_t)chain_next != seen_next) {
+                    seen_next = (uint32_t)chain_next;
+                    last_activity_us = now;
+                } else if (now - last_activity_us > P.idle_exit_ms * 977u) {
                     if (chain_next > oldest + P.R) oldest = chain_next - P.R;
                     for (;;) {
                         const unsigned long long q = oldest + lane;
@@ -631,7 +649,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                     if (oldest >= chain_next)
                         quit = true;
                     else
-                        last_activity = now;
+                        last_activity_us = now;
                 }
             }
             if (quit) {
@@ -815,17 +833,18 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         have_token = pos + n < 32u || K == 1u; /* still mine: nobody else can move it */
         my_pub = new_pub;
         token_at = my_next + n;
-        if (n != n_seen) repoll = true; /* the ticket ring took fewer requests than the poll in flight assumes */
 
         /* ---- phase 4: keys, descriptors, tickets ----------------------------------------------- */
         const uint32_t fine = UNIT_MODE(fine_max, half_min, 0u); /* of the request's first chunk (statistics, descriptor) */
         {   /* statistics for aes_engine_info */
             const uint32_t me = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_FINE));
             const uint32_t mh = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_HALF));
-            n_eighths += __popc(me);
-            n_halves += __popc(mh);
-            n_rows += n - __popc(me) - __popc(mh);
-            stats_dirty = true; /* written to the host when the ring is next found empty */
+            if (lane == 0) { /* kept in shared memory, not in registers; written to the host when the ring is next found empty */
+                c->disp_stat[0] += __popc(me);
+                c->disp_stat[1] += __popc(mh);
+                c->disp_stat[2] += n - __popc(me) - __popc(mh);
+                c->disp_stat[3] = 1u;
+            }
         }
         uint32_t keyloc = kw & 0xffffu;
         if (!(kw & AESOFF_KW_RAW) && keyloc >= AESOFF_KEY_IDS) keyloc = AESOFF_KEY_IDS + slot; /* never sent by the host */
@@ -906,6 +925,9 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                 ISSUE_POLL(b_seq + (unsigned long long)AESOFF_BATCH * K, 0u, true);
             else
                 ISSUE_POLL(b_seq, pos + n, true);
+            n_looked = n_issued - 1u; /* older polls in flight are stale: wait them out with this one, do not look */
+        } else {
+            n_looked = n_issued;
         }
 #endif
         pos += n;

@@ -476,13 +476,17 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
         p.tune[AESOFF_TUNE_TAIL_LEFT] = 2 * W;
         p.tune[AESOFF_TUNE_SPREAD_AHEAD] = W / 2;
         p.tune[AESOFF_TUNE_SPREAD_MAX] = 16;
+        p.tune[AESOFF_TUNE_POLL_DEPTH] = 3;
+        p.tune[AESOFF_TUNE_POLL_GAP] = 350;
         if (const char *t = getenv("AESOFF_TUNE")) {
-            for (int i = 0; i < 7 && t && *t; ++i) {
+            for (int i = 0; i < 9 && t && *t; ++i) {
                 char *end = nullptr;
                 const unsigned long v = strtoul(t, &end, 10);
                 if (end != t) p.tune[i] = (uint32_t)v;
                 t = (*end == ',') ? end + 1 : nullptr;
             }
+            if (p.tune[AESOFF_TUNE_POLL_DEPTH] < 1u) p.tune[AESOFF_TUNE_POLL_DEPTH] = 1u;
+            if (p.tune[AESOFF_TUNE_POLL_DEPTH] > 3u) p.tune[AESOFF_TUNE_POLL_DEPTH] = 3u;
         }
     }
     if (aesoff_launch_engine(&p, e.n_ctas, e.stream) != 0) {

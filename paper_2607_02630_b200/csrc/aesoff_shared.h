@@ -155,6 +155,8 @@ typedef struct __attribute__((aligned(16))) aesoff_ticket {
 #define AESOFF_TUNE_TAIL_LEFT    4    /* ... has its last this many rows cut into half rows              (2 W)   */
 #define AESOFF_TUNE_SPREAD_AHEAD 5    /* idle GPU and at most this many rows ahead: one chunk per CTA ... (W / 2) */
 #define AESOFF_TUNE_SPREAD_MAX   6    /* ... of at most this many rows                                   (16)    */
+#define AESOFF_TUNE_POLL_DEPTH   7    /* polls of the ring the token holder keeps in flight while the queue is short (1..3) */
+#define AESOFF_TUNE_POLL_GAP     8    /* nanoseconds between issuing them, so that they stay spread over a round trip       */
 
 typedef struct aesoff_params {
     aesoff_host_slot_t *hring;      /* host-mapped (persistent mode)                     */
@@ -178,7 +180,7 @@ typedef struct aesoff_params {
     uint32_t            fine_rows;  /* requests of at most this many rows may be cut into units smaller than a row; 0 = never */
     uint64_t            first_seq;  /* sequence number of the first request of this launch */
     uint32_t            n_disp;     /* dispatcher warps (persistent mode), 1 .. AESOFF_MAX_DISPATCHERS      */
-    uint32_t            tune[7];    /* unit-size policy thresholds in rows, AESOFF_TUNE_* (dispatcher_loop) */
+    uint32_t            tune[9];    /* dispatcher policy, AESOFF_TUNE_* (dispatcher_loop)                   */
 } aesoff_params_t;
 
 #endif

@@ -33,16 +33,37 @@ def cubin(tmp_path_factory):
     return out, p.stdout
 
 
-def test_engine_kernel_has_no_spills_and_96_registers(cubin):
-    _, log = cubin
+def test_engine_kernel_registers_and_spills(cubin):
+    """96 registers (18 warps per CTA: five warps on two of the four sub-partitions).  ptxas may park a few
+    loop-invariant words of the worker loop (slot addresses) in local memory and reload them once per unit, but nothing
+    may spill inside the cipher's round loops, and the dispatcher's polls no longer live in registers at all (they are
+    cp.async copies into shared memory: a spilled poll register used to undo the overlap of poll and processing)."""
+    path, log = cubin
     m = re.search(r"Compiling entry function '\S*aesoff_engine_kernel\S*' for 'sm_100a'.*?"
                   r"(\d+) bytes stack frame, (\d+) bytes spill stores, (\d+) bytes spill loads.*?Used (\d+) registers",
                   log, re.S)
     assert m, log
     stack, st, ld, regs = map(int, m.groups())
-    assert st == 0 and ld == 0, "the engine kernel spills (%d B stores, %d B loads): see this file's docstring" % (st, ld)
+    assert st <= 16 and ld <= 16, "the engine kernel spills %d B (stores) / %d B (loads)" % (st, ld)
     assert regs <= 96, regs
     assert stack <= 64, stack
+    exe = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(exe):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([exe, "-sass", path], stdout=subprocess.PIPE, text=True).stdout
+    ins = [(int(a, 16), t) for a, t in re.findall(r"/\*([0-9a-f]{4,})\*/\s+(.*?);", sass)]
+    index = {a: i for i, (a, _) in enumerate(ins)}
+    round_loops = 0
+    for i, (a, t) in enumerate(ins):
+        mm = re.search(r"BRA.*?0x([0-9a-f]+)", t)
+        if mm and int(mm.group(1), 16) < a and int(mm.group(1), 16) in index:
+            body = [x for _, x in ins[index[int(mm.group(1), 16)]:i + 1]]
+            if len(body) < 300 and sum("LDS" in x for x in body) >= 60:      # a main-round loop: 64 lookups per pass
+                round_loops += 1
+                assert not any(re.search(r"\b(LDL|STL)\b", x) for x in body), "local-memory traffic inside a round loop"
+                assert "cp.async" not in "".join(body)
+    assert round_loops >= 2
+    assert "LDGSTS" in sass                                                     # the polls: cp.async into shared memory
 
 
 def test_sass_has_the_instructions_the_design_rests_on(cubin):
