@@ -575,19 +575,26 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         const uint32_t *sw = c->stage[cur][lane];
         const uint32_t *ax = c->stage[cur][32];
         const uint32_t tag = (uint32_t)s;
-        uint32_t kw = sw[AESOFF_PW_INDEX(AESOFF_PW_KEY)];
-        bool valid = lane >= pos && sw[3] == tag && sw[7] == tag && sw[11] == tag && sw[15] == tag;
+        /* the first line of the descriptor in four 16-byte reads, kept in registers for the whole take: under load the
+         * dispatcher's shared-memory reads queue behind its SM's table lookups, so there are few of them
+         * (pieces: {ICB0..2} {ICB3, src} {dst, len lo} {len hi, key word, mode}, each with its tag) */
+        const uint4 p0 = *reinterpret_cast<const uint4 *>(sw + 0), p1 = *reinterpret_cast<const uint4 *>(sw + 4);
+        const uint4 p2 = *reinterpret_cast<const uint4 *>(sw + 8), p3 = *reinterpret_cast<const uint4 *>(sw + 12);
+        const uint32_t kw = p3.y;
+        bool valid = lane >= pos && p0.w == tag && p1.w == tag && p2.w == tag && p3.w == tag;
         if (valid && (kw & AESOFF_KW_RAW)) valid = sw[19] == tag && sw[23] == tag && sw[27] == tag && sw[31] == tag;
         const uint32_t vrun = ~(__ballot_sync(0xffffffffu, valid) >> pos); /* bit i: request pos + i is not ready */
         uint32_t n = vrun ? (uint32_t)(__ffs(vrun) - 1) : 32u;           /* length of the ready run from pos */
         if (n > 32u - pos) n = 32u - pos;
-        const uint32_t stop = ax[AUX_CTL + AESOFF_CTL_STOP];
-        unsigned long long chain_pub = ((unsigned long long)ax[AUX_CHAIN + 1] << 32) | ax[AUX_CHAIN];
-        unsigned long long chain_next = ((unsigned long long)ax[AUX_CHAIN + 3] << 32) | ax[AUX_CHAIN + 2];
-        const unsigned long long reserved = ((unsigned long long)ax[AUX_TKT + 1] << 32) | ax[AUX_TKT];
-        const unsigned long long idle = ((unsigned long long)ax[AUX_IDLE + 1] << 32) | ax[AUX_IDLE];
-        const uint32_t quit_word = ax[AUX_IDLE + 2];
-        queue_long = ax[AUX_IDLE + 3] != 0u;
+        const uint4 a_ctl = *reinterpret_cast<const uint4 *>(ax + AUX_CTL), a_chain = *reinterpret_cast<const uint4 *>(ax + AUX_CHAIN);
+        const uint4 a_tkt = *reinterpret_cast<const uint4 *>(ax + AUX_TKT), a_idle = *reinterpret_cast<const uint4 *>(ax + AUX_IDLE);
+        const uint32_t stop = a_ctl.x; /* AESOFF_CTL_STOP is word 0 */
+        unsigned long long chain_pub = ((unsigned long long)a_chain.y << 32) | a_chain.x;
+        unsigned long long chain_next = ((unsigned long long)a_chain.w << 32) | a_chain.z;
+        const unsigned long long reserved = ((unsigned long long)a_tkt.y << 32) | a_tkt.x;
+        const unsigned long long idle = ((unsigned long long)a_idle.y << 32) | a_idle.x;
+        const uint32_t quit_word = a_idle.z;
+        queue_long = a_idle.w != 0u;
         token_at = chain_next;
         wide = (n >= 8u) ? 1u : 0u;
         const uint32_t n_seen = n;
@@ -673,9 +680,9 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         uint32_t rows = 0;
 #define PW(p) sw[AESOFF_PW_INDEX(p)]
         if (mine) {
-            const unsigned long long len = ((unsigned long long)PW(AESOFF_PW_LEN + 1) << 32) | PW(AESOFF_PW_LEN);
+            const unsigned long long len = ((unsigned long long)p3.x << 32) | p2.z;
             const unsigned long long nblocks = (len >> 4) + ((len & 15ull) ? 1ull : 0ull);
-            const uint32_t c0 = (PW(AESOFF_PW_SPARE) & 3u) ? 0u : PW(AESOFF_PW_ICB + 3) >> 24; /* rows start at counter byte 0 */
+            const uint32_t c0 = (p3.z & 3u) ? 0u : p1.x >> 24; /* rows start at counter byte 0 (CTR) or at the payload's start */
             rows = nblocks ? (uint32_t)((nblocks + c0 + AESOFF_ROW_BLOCKS - 1) >> 8) : 0u;
         }
         /* rows of this poll up to and including request k */
@@ -821,10 +828,6 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             asm volatile("st.volatile.global.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(g_chain), "r"((uint32_t)new_pub),
                          "r"((uint32_t)(new_pub >> 32)), "r"((uint32_t)nx), "r"((uint32_t)(nx >> 32))
                          : "memory");
-            /* what the service warps read.  Not a store: a dispatcher that got the token later may already
-             * have published a larger count.  No fence: the count only tells the service warps how many tickets
-             * they may reserve; a ticket is taken when its own 16-byte word shows up (tag).                  */
-            if (total) atomicMax(g_published, new_pub);
         }
         if (K > 1u && (wide != 0u) != queue_long) { /* as the holder: tell the others whether reading ahead pays */
             queue_long = wide != 0u;
@@ -865,10 +868,10 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             /* the 24 descriptor words as 8 pieces of {3 words, tag}: see aesoff_dq_entry_t */
             uint4 *d4 = reinterpret_cast<uint4 *>(P.dq + slot);
             const uint32_t tg = (uint32_t)s;
-            d4[0] = make_uint4(PW(AESOFF_PW_ICB + 0), PW(AESOFF_PW_ICB + 1), PW(AESOFF_PW_ICB + 2), tg);
-            d4[1] = make_uint4(PW(AESOFF_PW_ICB + 3), PW(AESOFF_PW_SRC), PW(AESOFF_PW_SRC + 1), tg);
-            d4[2] = make_uint4(PW(AESOFF_PW_DST), PW(AESOFF_PW_DST + 1), PW(AESOFF_PW_LEN), tg);
-            d4[3] = make_uint4(PW(AESOFF_PW_LEN + 1), kw >> 24, PW(AESOFF_PW_SPARE) & 3u, tg);
+            d4[0] = p0; /* the first three pieces as they came (their tag is this request's) */
+            d4[1] = p1;
+            d4[2] = p2;
+            d4[3] = make_uint4(p3.x, kw >> 24, p3.z & 3u, tg);
             d4[4] = make_uint4(nchunks, 1u << clog, (uint32_t)s, tg);
             d4[5] = make_uint4((uint32_t)(s >> 32), rows, 0u, tg);
             d4[6] = make_uint4((uint32_t)first_ticket, (uint32_t)(first_ticket >> 32), keyloc, tg);
@@ -906,6 +909,10 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         }
 #undef UNIT_MODE
         __syncwarp();
+        /* What the service warps read, raised once the tickets are on their way.  Not a store: a dispatcher that got
+         * the token later may already have published a larger count.  No fence: the count only tells the service warps
+         * how many tickets they may reserve; a ticket is taken when its own 16-byte word shows up (tag).          */
+        if (lane == 0 && total) atomicMax(g_published, new_pub);
         /* an empty request (len == 0) has no ticket: complete it here */
         if (take && nchunks == 0) {
             __threadfence_system();
