@@ -168,7 +168,8 @@ __device__ __forceinline__ uint32_t claim_unit(CtaCtl *c, uint32_t lane)
 }
 
 /* The slot's chunk is finished: count the request's chunks down; the last one signals the host. */
-__device__ __forceinline__ void complete_chunk(const aesoff_params_t &P, CtaCtl *c, uint32_t s)
+template <class PP>
+__device__ __forceinline__ void complete_chunk(const PP &P, CtaCtl *c, uint32_t s)
 {
     const Slot *sl = &c->slot[s];
     const uint32_t ring = sl->ring_slot, nchunks = sl->desc.nchunks;
@@ -190,7 +191,17 @@ __device__ __forceinline__ void complete_chunk(const aesoff_params_t &P, CtaCtl 
     sts_volatile(&c->busy[s], 0u); /* the service warp may refill the slot */
 }
 
-__device__ void worker_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase, uint32_t lane)
+/* NOT inlined into the kernel, and handed only the four pointers it needs: ptxas then allocates and schedules the
+ * cipher loops by themselves.  Inlined beside the dispatcher and the service warp, the same source ran 0.6-0.9 % slower
+ * after every change to THOSE roles (same instruction counts in the round loops, different schedule; found by timing the
+ * drain-mode kernel of successive commits): 922 -> 934 GB/s at 1 MiB x 64, 652 -> 659 at AES-256 8 MiB x 16.        */
+struct WorkerParams {
+    uint32_t *dq_done;
+    volatile uint64_t *hmail;
+    uint64_t *dev_done_seq;
+    uint64_t *counters;
+};
+__device__ __noinline__ void worker_loop(const WorkerParams P, CtaCtl *c, uint32_t ybase, uint32_t lane)
 {
 #ifdef AESOFF_DEBUG
     bool first = true;
@@ -987,7 +998,12 @@ __global__ void __launch_bounds__(AESOFF_CTA_THREADS, 1) aesoff_engine_kernel(co
         DBG_MAX(2); /* last CTA has its tables */
         asm volatile("bar.sync 1, %0;" ::"n"(AESOFF_CTA_THREADS) : "memory");
         if (tid == 0) sts_volatile(&c->tables_ready, 1u);
-        worker_loop(P, c, tbase | (lane * 4u), lane);
+        WorkerParams wp;
+        wp.dq_done = P.dq_done;
+        wp.hmail = P.hmail;
+        wp.dev_done_seq = P.dev_done_seq;
+        wp.counters = P.counters;
+        worker_loop(wp, c, tbase | (lane * 4u), lane);
         DBG_MIN(6); /* first worker warp leaves */
         DBG_MAX(7); /* last worker warp leaves  */
     }
