@@ -50,8 +50,7 @@ struct __align__(16) Slot {
     uint32_t n_rows;        /* rows of this chunk                                               */
     uint32_t mode;          /* AESOFF_MODE_CTR / _ECB_ENC / _ECB_DEC / _CBC_DEC                 */
     uint32_t pad_[2];
-    uint32_t fine;          /* unit size: 0 rows (AESOFF_ROWS_PER_UNIT of them), AESOFF_FLAG_HALF half a row (128 blocks),
-                               AESOFF_FLAG_FINE one k-iteration of a row (32 blocks)            */
+    uint32_t pad2_;         /* (the unit size lives in CtaCtl::unit_mode)                       */
 };                          /* 384 B */
 
 struct __align__(16) CtaCtl {
@@ -63,6 +62,10 @@ struct __align__(16) CtaCtl {
     uint32_t done[AESOFF_SLOTS];  /* units finished                                              */
     uint32_t stamp[AESOFF_SLOTS]; /* fill order, so that workers take the oldest open slot first */
     uint32_t busy[AESOFF_SLOTS];  /* 0 free, 1 filled and not yet completed                      */
+    /* unit size of the slot's chunk: 0 rows (AESOFF_ROWS_PER_UNIT of them), AESOFF_FLAG_HALF, AESOFF_FLAG_FINE.  An array of
+     * its own because the service warp reads it lane by lane for what the CTA holds: as a field of Slot (384 bytes apart,
+     * i.e. one bank) that one load was a 16-way bank conflict and 1.2 % of the SM's shared-memory wavefronts (ncu, source page). */
+    uint32_t unit_mode[AESOFF_SLOTS];
     uint32_t exit_flag;
     uint32_t disp_stat[4];        /* dispatcher: requests cut into 1/8 rows / half rows / rows so far, and "changed" */
     uint32_t tables_ready;        /* set by a worker once the tables are filled: the service warp, which starts fetching
@@ -225,7 +228,7 @@ __device__ __noinline__ void worker_loop(const WorkerParams P, CtaCtl *c, uint32
         uint8_t *dst = reinterpret_cast<uint8_t *>(sl->desc.dst);
         const CtrGeom g = ctr_geom(sl->desc.icb[0], sl->desc.icb[1], sl->desc.icb[2], sl->desc.icb[3]);
         const uint32_t n_units = sl->n_units;
-        const uint32_t fine = sl->fine;
+        const uint32_t fine = c->unit_mode[s];
         if (sl->mode != AESOFF_MODE_CTR) {
             /* ECB / CBC-decrypt: the same units over rows of 256 blocks, no counter (the ICB words hold the IV) */
             const uint4 iv = make_uint4(sl->desc.icb[0], sl->desc.icb[1], sl->desc.icb[2], sl->desc.icb[3]);
@@ -330,7 +333,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
             if (mine && !is_free) {
                 const uint32_t w = lds_volatile(&c->claim[lane]);
                 const uint32_t left = (w >> 16) > (w & 0xffffu) ? (w >> 16) - (w & 0xffffu) : 0u;
-                const uint32_t f = c->slot[lane].fine;
+                const uint32_t f = c->unit_mode[lane];
                 held = (f & AESOFF_FLAG_FINE) ? left : (f & AESOFF_FLAG_HALF) ? left * 4u : left * 8u * AESOFF_ROWS_PER_UNIT;
             } else if (have) {
                 held = per_ticket;
@@ -449,7 +452,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
                 sl->unit0_row = (uint32_t)row0;
                 sl->ring_slot = ring;
                 sl->n_units = n_units;
-                sl->fine = fine;
+                c->unit_mode[lane] = fine;
                 sl->mode = sl->desc.flags & 3u;
                 c->done[lane] = 0u;
                 c->stamp[lane] = stamp_base + __popc(ready_mask & ((1u << lane) - 1u));
