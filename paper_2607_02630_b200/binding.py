@@ -315,6 +315,31 @@ def aes_loop_run(nonces, srcs, dsts, lens, window: int, ctx: int = 0, keys=None,
     return out
 
 
+def aes_loop_prepare(nonces, srcs, dsts, lens, window: int, ctx: int, repeat: int = 1, mode: int = 0):
+    """Marshals a closed-loop run over a shared context ONCE and returns a function that runs it (aes_loop_run in
+    aesoff.h) and returns (elapsed_ns, bytes, requests): for callers that repeat the same batch, e.g. bench.py's timed
+    steps, so that no per-step Python marshalling sits inside a timed region.  The arrays are kept alive by the closure."""
+    n = len(lens)
+    a_src, a_dst, a_len = _ptr_array(srcs), _ptr_array(dsts), _ptr_array(lens)
+    a_non = np.ascontiguousarray(np.asarray(nonces, dtype=np.uint8)).reshape(-1)
+    assert a_non.size == 16 * n
+    spec = aes_loop_spec_t()
+    spec.n, spec.window, spec.repeat, spec.ctx, spec.mode = n, window, repeat, ctx, mode
+    spec.nonces, spec.srcs, spec.dsts, spec.lens = a_non.ctypes.data, a_src.ctypes.data, a_dst.ctypes.data, a_len.ctypes.data
+    res = aes_loop_result_t()
+    p_spec, p_res, run = ctypes.byref(spec), ctypes.byref(res), _lib.aes_loop_run
+    keep = (a_src, a_dst, a_len, a_non, spec, res)
+
+    def go():
+        rc = run(p_spec, p_res, None)
+        if rc != AES_OK:
+            raise AesOffError(rc, "aes_loop_run")
+        return res.elapsed_ns, res.bytes, res.requests
+
+    go.keep = keep
+    return go
+
+
 def aes_openloop_run(nonces, srcs, dsts, lens, arrival_ns, ctx: int, blocking: bool = False) -> dict:
     """Runs the native open loop (see aes_openloop_run in aesoff.h): request i is submitted once
     arrival_ns[i] has passed.  Returns elapsed_ns, bytes, requests, ring_full_spins, max_in_flight, lat_ns."""
