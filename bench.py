@@ -397,6 +397,17 @@ def main():
         torch.cuda.synchronize()
         t1 = time.perf_counter() if args.backend != "engine" else t1h
     barrier()
+    worker_stats = None
+    if args.backend == "engine":
+        # -DAESOFF_WSTATS builds only (AESOFF_NVCC_EXTRA=-DAESOFF_WSTATS python -m paper_2607_02630_b200.build --force): what the
+        # worker warps of the persistent engine did during the K timed steps, from their own clock64 counters
+        import ctypes
+
+        ws = (ctypes.c_uint64 * 3)()
+        if B._lib.aesoff_debug_worker_stats(local_rank, ws) == 0 and ws[2]:
+            worker_stats = {"in_units_frac": ws[0] / float(ws[0] + ws[1]), "waiting_between_units_frac": ws[1] / float(ws[0] + ws[1]),
+                            "units": int(ws[2]), "clocks_per_unit": ws[0] / float(ws[2]),
+                            "how": "clock64 per worker warp: inside units / between two units, first unit to last unit of the engine run"}
     gpu_launches = B.aes_engine_info()["kernel_launches"] - launches_before
     ms_dev = ev0.elapsed_time(ev1)
     ms_host = 1e3 * (t1 - t0)
@@ -453,7 +464,7 @@ def main():
                    "l2": "inputs larger than L2 (%.1f GiB src + same dst per step)" % (n * size / 2**30),
                    "seed": workloads.SEED_BASE + w.config_index},
         "gpu_launches": int(gpu_launches), "ms_host": ms_host, "engine_start_ms": engine_start_ms,
-        "verified_vs_oracle": verified, "verified_bytes": verified_bytes,
+        "verified_vs_oracle": verified, "verified_bytes": verified_bytes, "worker_stats": worker_stats,
         "clocks": clk, "roofline": roofline,
     }
 

@@ -209,8 +209,26 @@ __device__ __noinline__ void worker_loop(const WorkerParams P, CtaCtl *c, uint32
 #ifdef AESOFF_DEBUG
     bool first = true;
 #endif
+#ifdef AESOFF_WSTATS
+    /* -DAESOFF_WSTATS builds: per worker warp, clocks inside units and clocks between two units (waiting for work), so that
+     * the persistent engine's own occupancy is measured, not extrapolated from a launch (aesoff_debug_worker_stats) */
+    long long ws_busy = 0, ws_wait = 0, ws_prev = 0;
+    unsigned long long ws_units = 0;
+#endif
     for (;;) {
         const uint32_t got = claim_unit(c, lane);
+#ifdef AESOFF_WSTATS
+        const long long ws_t1 = clock64();
+        if (got == CLAIM_EXIT) {
+            if (lane == 0) {
+                atomicAdd(reinterpret_cast<unsigned long long *>(P.counters) + AESOFF_CNT_DEBUG + 0, (unsigned long long)ws_busy);
+                atomicAdd(reinterpret_cast<unsigned long long *>(P.counters) + AESOFF_CNT_DEBUG + 1, (unsigned long long)ws_wait);
+                atomicAdd(reinterpret_cast<unsigned long long *>(P.counters) + AESOFF_CNT_DEBUG + 2, ws_units);
+            }
+            break;
+        }
+        if (ws_units) ws_wait += ws_t1 - ws_prev;
+#endif
         if (got == CLAIM_EXIT) break;
 #ifdef AESOFF_DEBUG
         if (lane == 0 && first) {
@@ -272,6 +290,11 @@ __device__ __noinline__ void worker_loop(const WorkerParams P, CtaCtl *c, uint32
             if (d + 1 == n_units) complete_chunk(P, c, s);
         }
         __syncwarp();
+#ifdef AESOFF_WSTATS
+        ws_prev = clock64();
+        ws_busy += ws_prev - ws_t1;
+        ++ws_units;
+#endif
     }
 }
 

@@ -636,6 +636,14 @@ extern "C" int aes_engine_info(aes_engine_info_t *out)
     return aes_engine_info_device(pick, out);
 }
 
+/* -DAESOFF_WSTATS builds: {clocks inside units, clocks waiting between units, units} summed over all worker warps of the
+ * engine run that was stopped last on `device` (read after aes_engine_stop); zeros otherwise.  Tuning aid, not in aesoff.h. */
+extern "C" __attribute__((visibility("default"))) int aesoff_debug_worker_stats(int device, uint64_t out[3])
+{
+    if (device < 0 || device >= AESOFF_MAX_DEVICES || !g_engs[device].counters) return -1;
+    return cudaMemcpy(out, g_engs[device].counters + AESOFF_CNT_DEBUG, 24, cudaMemcpyDeviceToHost) == cudaSuccess ? 0 : -1;
+}
+
 /* AESOFF_DISP_STATS builds: per-dispatcher counters (polls that took requests, requests, token wait and work
  * in units of 64 ns, empty polls), 5 words per dispatcher; zeros otherwise.  Tuning aid, not in aesoff.h.   */
 extern "C" __attribute__((visibility("default"))) int aesoff_debug_dispatch_stats(uint32_t out[5 * AESOFF_MAX_DISPATCHERS])

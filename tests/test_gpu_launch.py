@@ -211,3 +211,39 @@ def test_consecutive_rows_and_carries_out_of_counter_byte_14(P, low4):
         gots.append(dst[s0:e0].cpu().numpy())
     for s0, got, want in zip(starts, gots, G.oracle_many(jobs)):
         assert G.first_mismatch(got, want) == -1, "window at %d" % s0
+
+
+def test_launches_on_two_streams_do_not_trample_each_other(P):
+    """aes_ctr_launch_batch keeps ONE device blob of descriptors, keys and tickets; calls on different streams are
+    serialised on the device through an event (the second call's copy waits for the first call's kernel).  Two streams
+    alternating, several calls each, nothing synchronised in between; every byte against the oracle."""
+    import gpu_util as G
+
+    torch = G.torch_cuda()
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 6900]))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    keys = [rng.bytes(16), rng.bytes(32)]
+    ctxs = [P.aes_ctx_create(k) for k in keys]
+    calls = []
+    for c in range(8):
+        n = 3 + c % 3
+        datas = [np.frombuffer(rng.bytes(int(rng.integers(1, 300000))), dtype=np.uint8) for _ in range(n)]
+        icbs = [rng.bytes(16) for _ in range(n)]
+        srcs = [G.to_device(d) for d in datas]
+        dsts = [G.device_empty(len(d)) for d in datas]
+        calls.append((c % 2, datas, icbs, srcs, dsts))
+    torch.cuda.synchronize()
+    for which, datas, icbs, srcs, dsts in calls:
+        P.aes_ctr_launch_batch([ctxs[which]] * len(datas), b"".join(icbs), [s.data_ptr() for s in srcs],
+                               [d.data_ptr() for d in dsts], [len(d) for d in datas], cuda_stream=streams[which].cuda_stream)
+    for s in streams:
+        s.synchronize()
+    jobs, gots = [], []
+    for which, datas, icbs, srcs, dsts in calls:
+        for d, i, out in zip(datas, icbs, dsts):
+            jobs.append((keys[which], i, d))
+            gots.append(out.cpu().numpy()[:len(d)])
+    for k, (got, want) in enumerate(zip(gots, G.oracle_many(jobs))):
+        assert G.first_mismatch(got, want) == -1, "request %d" % k
+    for c in ctxs:
+        P.aes_ctx_destroy(c)
