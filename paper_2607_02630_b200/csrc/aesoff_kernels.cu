@@ -313,6 +313,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
     unsigned long long t = 0;   /* that ticket */
     uint32_t stamp_base = 0;
     bool counted_idle = false;  /* this CTA is included in the device-wide idle-CTA count */
+    uint32_t last_chunk_rows = P.chunk_rows; /* rows of the chunk this CTA read last (requests choose their chunk size) */
 
     for (;;) {
         const bool is_free = mine && lds_volatile(&c->busy[lane]) == 0u;
@@ -351,7 +352,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
          *    to hide a refill (microseconds against 10 us per row), little enough that the end of a
          *    burst is not left to the few CTAs that grabbed 16 chunks each.                        */
         {
-            const uint32_t per_ticket = P.chunk_rows * 8u;
+            const uint32_t per_ticket = last_chunk_rows * 8u; /* a reserved ticket that has not been read yet: as large as the last one */
             uint32_t held = 0;
             if (mine && !is_free) {
                 const uint32_t w = lds_volatile(&c->claim[lane]);
@@ -462,10 +463,12 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
                 }
             }
             __syncwarp();
+            uint32_t seen_rows = 0;
             if (ready) {
                 Slot *sl = &c->slot[lane];
                 const unsigned long long rows = sl->desc.rows;
                 const uint32_t crows = sl->desc.chunk_rows;
+                seen_rows = crows;
                 const unsigned long long row0 = (unsigned long long)chunk * crows;
                 const uint32_t nrows = (uint32_t)((rows - row0) < crows ? (rows - row0) : crows);
                 const uint32_t fine = unit_mode & (AESOFF_FLAG_FINE | AESOFF_FLAG_HALF);
@@ -485,6 +488,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
                 have = false;
             }
             stamp_base += __popc(ready_mask);
+            last_chunk_rows = __reduce_max_sync(0xffffffffu, seen_rows); /* ready_mask != 0: at least one lane saw one */
             continue;
         }
 
@@ -788,6 +792,11 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                  * hold is counted in chunk_rows-sized tickets (service_loop) */
                 clog = 0;
                 while ((gridDim.x << clog) < rows) ++clog;
+            } else if (mine && may_cut && rows >= 4u * gridDim.x * AESOFF_WORKER_WARPS) {
+                /* a very long request (37 MiB and up): 16-row chunks, a quarter of the tickets -- cut into 4-row chunks a lone
+                 * 64 MiB request ran at 747 GB/s, the service warps' ticket and descriptor traffic being what held it back;
+                 * with 16-row chunks 789.  (What a CTA may hold is counted in rows of the chunks it has seen: service_loop.) */
+                clog = max(clog, 4u);
             }
             int fm = -1, hm = 0x7fffffff;
             if (may_cut) {
