@@ -797,6 +797,8 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                  * 64 MiB request ran at 747 GB/s, the service warps' ticket and descriptor traffic being what held it back;
                  * with 16-row chunks 789.  (What a CTA may hold is counted in rows of the chunks it has seen: service_loop.) */
                 clog = max(clog, 4u);
+            } else if (mine && may_cut && rows >= 64u && total_q >= 4u * gridDim.x * AESOFF_WORKER_WARPS) {
+                clog = max(clog, 3u); /* saturation: 8-row chunks, half the slot fills (8 MiB x 16: 938 -> 942 GB/s, AES-256 661 -> 664) */
             }
             int fm = -1, hm = 0x7fffffff;
             if (may_cut) {
