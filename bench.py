@@ -854,6 +854,17 @@ def extras(args, B, torch, dev, local_rank, w, keybits, ctx, srcs, dsts, lens, s
                               "payload_gbs": gbs, "lds_frac": gbs * lds_per_payload_byte / lds_peak,
                               "hbm_frac": 2 * gbs / hbm_peak, "launches_timed": len(evs)}
 
+    # ---- the same batch as ONE closed loop over 10 passes: the window never drains between passes (a timed step above is
+    #      the whole 1,000-request job, so it fills an idle GPU and drains it every time: DESIGN.md R14) ----
+    if args.backend == "engine":
+        B.aes_engine_start(local_rank, chunk_rows=args.chunk_rows, idle_exit_ms=30000)
+        go = B.aes_loop_prepare(w.icb, srcs, dsts, lens, window=w.in_flight, ctx=ctx, repeat=10)
+        go()
+        el, by, _ = go()
+        B.aes_engine_stop()
+        res["steady_state"] = {"payload_gbs": by / el, "lds_frac": by / el * lds_per_payload_byte / lds_peak, "hbm_frac": 2 * by / el / hbm_peak,
+                               "how": "the %d requests of the step, 10 passes back to back in one closed loop, %d in flight throughout" % (n, w.in_flight)}
+
     # ---- e2e: payloads in pinned HOST memory, read and written by the kernel over PCIe ----
     n_e2e = min(n, 256)
     hs = B.aes_host_alloc(n_e2e * size)
