@@ -346,7 +346,6 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
          *    CTA of the persistent engine also keeps ONE reservation on a ticket that does not
          *    exist yet, so that a lone request finds 148 CTAs waiting, one ticket each.         */
         unsigned long long avail = pub > tk ? pub - tk : 0ull;
-        if (persistent && busy_mask == 0u && have_mask == 0u && avail == 0ull) avail = 1ull;
         /*    A CTA does not hoard: what it holds (unclaimed units of its open slots plus the tickets
          *    it has reserved, in 1/8-row units) stays near one and a half rows per worker -- enough
          *    to hide a refill (microseconds against 10 us per row), little enough that the end of a
@@ -363,6 +362,12 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
                 held = per_ticket;
             }
             held = __reduce_add_sync(0xffffffffu, held);
+            /* The reservation on a ticket that does not exist yet: an idle CTA keeps one, and so does a CTA whose workers
+             * are nearly out of work (less than half a row each): the ticket is then picked up one L2 round trip after it
+             * is written instead of three (see the count, reserve, poll), which is latency that a window of small requests
+             * turns into throughput.                                                                                  */
+            if (persistent && avail == 0ull && have_mask == 0u && (busy_mask == 0u || held < AESOFF_WORKER_WARPS * P.tune[AESOFF_TUNE_PRERESERVE]))
+                avail = 1ull;
             const uint32_t hold_max = AESOFF_WORKER_WARPS * 12u; /* 1.5 rows per worker */
             unsigned long long cap = held < hold_max ? (hold_max - held + per_ticket - 1u) / per_ticket : 0u;
             if (cap == 0ull && busy_mask == 0u && have_mask == 0u) cap = 1ull;

@@ -478,8 +478,9 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
         p.tune[AESOFF_TUNE_SPREAD_MAX] = 16;
         p.tune[AESOFF_TUNE_POLL_DEPTH] = 3;
         p.tune[AESOFF_TUNE_POLL_GAP] = 350;
+        p.tune[AESOFF_TUNE_PRERESERVE] = 4;
         if (const char *t = getenv("AESOFF_TUNE")) {
-            for (int i = 0; i < 9 && t && *t; ++i) {
+            for (int i = 0; i < 10 && t && *t; ++i) {
                 char *end = nullptr;
                 const unsigned long v = strtoul(t, &end, 10);
                 if (end != t) p.tune[i] = (uint32_t)v;

@@ -156,6 +156,7 @@ typedef struct __attribute__((aligned(16))) aesoff_ticket {
 #define AESOFF_TUNE_SPREAD_AHEAD 5    /* idle GPU and at most this many rows ahead: one chunk per CTA ... (W / 2) */
 #define AESOFF_TUNE_SPREAD_MAX   6    /* ... of at most this many rows                                   (16)    */
 #define AESOFF_TUNE_POLL_DEPTH   7    /* polls of the ring the token holder keeps in flight while the queue is short (1..3) */
+#define AESOFF_TUNE_PRERESERVE   9    /* a CTA holding less than this many 1/8 rows per worker keeps a reservation on a ticket that does not exist yet */
 #define AESOFF_TUNE_POLL_GAP     8    /* nanoseconds between issuing them, so that they stay spread over a round trip       */
 
 typedef struct aesoff_params {
@@ -180,7 +181,7 @@ typedef struct aesoff_params {
     uint32_t            fine_rows;  /* requests of at most this many rows may be cut into units smaller than a row; 0 = never */
     uint64_t            first_seq;  /* sequence number of the first request of this launch */
     uint32_t            n_disp;     /* dispatcher warps (persistent mode), 1 .. AESOFF_MAX_DISPATCHERS      */
-    uint32_t            tune[9];    /* dispatcher policy, AESOFF_TUNE_* (dispatcher_loop)                   */
+    uint32_t            tune[10];    /* dispatcher policy, AESOFF_TUNE_* (dispatcher_loop)                   */
 } aesoff_params_t;
 
 #endif
