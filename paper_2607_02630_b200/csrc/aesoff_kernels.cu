@@ -936,9 +936,10 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         if (__any_sync(0xffffffffu, take && (kw & AESOFF_KW_RAW))) __threadfence();
         __syncwarp();
         /* a request of up to eight chunks (the fine-grained regime: every request of the poll) gets its
-         * tickets from its own lane; the warp then shares out the long ones, 32 tickets per step */
-        if (take) {
-            for (uint32_t ch = 0; ch < nchunks && ch < 8u; ++ch) {
+         * tickets from its own lane; the warp then shares out the long ones, 32 tickets per step (all of their
+         * tickets: the per-lane loop costs the warp as many passes as its longest request has chunks) */
+        if (take && nchunks <= 8u) {
+            for (uint32_t ch = 0; ch < nchunks; ++ch) {
                 const unsigned long long tno = first_ticket + ch;
                 const uint32_t md = UNIT_MODE(fine_max, half_min, ch << clog) << AESOFF_TICKET_MODE_SHIFT;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
@@ -953,7 +954,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             const uint32_t cl = __shfl_sync(0xffffffffu, clog, k);
             const uint32_t fm = __shfl_sync(0xffffffffu, fine_max, k), hm = __shfl_sync(0xffffffffu, half_min, k);
             const uint32_t sq = (uint32_t)(b_seq + k);
-            for (uint32_t ch = 8u + lane; ch < nc; ch += 32) {
+            for (uint32_t ch = lane; ch < nc; ch += 32) {
                 const unsigned long long tno = ft + ch;
                 const uint32_t md = UNIT_MODE(fm, hm, ch << cl) << AESOFF_TICKET_MODE_SHIFT;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
