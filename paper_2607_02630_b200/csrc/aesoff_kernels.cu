@@ -742,26 +742,11 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         }
         const uint32_t rows_poll = __shfl_sync(0xffffffffu, rows_incl, n > 1 ? 31 : (int)pos);
 
-        /* ---- phase 3: the token -------------------------------------------------------------------- */
         const unsigned long long my_next = b_seq + pos;
-        if (have_token) {
-            chain_pub = my_pub;
-        } else {
-            /* only the token is read again: the load figures of the poll are heuristics, and the line the
-             * ticket counter lives on belongs to the service warps' atomics */
-            while (chain_next != my_next) {
-                uint4 v = make_uint4(0, 0, 0, 0);
-                if (lane == 0) v = ld_volatile_v4(P.counters + AESOFF_CNT_CHAIN);
-                chain_pub = ((unsigned long long)__shfl_sync(0xffffffffu, v.y, 0) << 32) | __shfl_sync(0xffffffffu, v.x, 0);
-                chain_next = ((unsigned long long)__shfl_sync(0xffffffffu, v.w, 0) << 32) | __shfl_sync(0xffffffffu, v.z, 0);
-            }
-        }
-        const unsigned long long published = chain_pub;
-#ifdef AESOFF_DISP_STATS
-        const unsigned long long dbg_t1 = globaltimer_ns();
-        dbg_wait += dbg_t1 - dbg_t0;
-        ++dbg_takes;
-#endif
+        /* the published count as this poll saw it (the reserved count and the idle CTAs come from the same poll): the
+         * load figures are heuristics, and sizing the requests BEFORE the token arrives keeps the token's holding time
+         * -- the one serial step of the dispatchers -- down to a sum, a ballot and a store */
+        const unsigned long long pub_est = have_token ? my_pub : chain_pub;
         /* Unit and chunk sizes by the load the request meets (all in 4 KiB rows; W = worker warps of the grid):
          *   backlog   rows published and not yet reserved by any CTA (chunk_rows per ticket, roughly)
          *   ahead     backlog + the rows of the requests before it in this poll
@@ -785,7 +770,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
          * on this path are 0.2 us on every request, so chunk sizes are powers of two and nothing here divides) */
         uint32_t nchunks = 0, clog = P.chunk_log2; /* rows per chunk = 1 << clog */
         {
-            const unsigned long long bl = (published > reserved ? published - reserved : 0ull) << P.chunk_log2;
+            const unsigned long long bl = (pub_est > reserved ? pub_est - reserved : 0ull) << P.chunk_log2;
             const uint32_t backlog = bl > 0x3fffffffull ? 0x3fffffffu : (uint32_t)bl;
             const uint32_t total_q = min(backlog + min(rows_poll, 0x3fffffffu), 0x3fffffffu);
             const uint32_t ahead = min(backlog + (rows_incl - rows), 0x3fffffffu);
@@ -833,6 +818,26 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                 if ((int)lane >= dd) incl += y;
             }
         }
+        /* ---- phase 3: the token -------------------------------------------------------------------- */
+        /* (everything above ran while it was on its way: what its holder still does is a sum, a ballot and a store) */
+        if (have_token) {
+            chain_pub = my_pub;
+        } else {
+            /* only the token is read again: the load figures of the poll are heuristics, and the line the
+             * ticket counter lives on belongs to the service warps' atomics */
+            while (chain_next != my_next) {
+                uint4 v = make_uint4(0, 0, 0, 0);
+                if (lane == 0) v = ld_volatile_v4(P.counters + AESOFF_CNT_CHAIN);
+                chain_pub = ((unsigned long long)__shfl_sync(0xffffffffu, v.y, 0) << 32) | __shfl_sync(0xffffffffu, v.x, 0);
+                chain_next = ((unsigned long long)__shfl_sync(0xffffffffu, v.w, 0) << 32) | __shfl_sync(0xffffffffu, v.z, 0);
+            }
+        }
+        const unsigned long long published = chain_pub;
+#ifdef AESOFF_DISP_STATS
+        const unsigned long long dbg_t1 = globaltimer_ns();
+        dbg_wait += dbg_t1 - dbg_t0;
+        ++dbg_takes;
+#endif
         const unsigned long long first_ticket = published + incl - nchunks;
         /* ticket-ring capacity: every unfinished ticket must stay within TM of the newest.  `base`
          * is only refreshed (32 completion words per L2 round trip) when the cached one says no. */
