@@ -70,7 +70,8 @@ struct __align__(16) CtaCtl {
     uint32_t disp_stat[4];        /* dispatcher: requests cut into 1/8 rows / half rows / rows so far, and "changed" */
     uint32_t tables_ready;        /* set by a worker once the tables are filled: the service warp, which starts fetching
                                      tickets while they are being built, needs them for a decrypting request's keys */
-    uint32_t pad[2];
+    uint32_t token_moved_us;      /* dispatcher: when it last saw the token move (1.024 us units; kept here, not in a register) */
+    uint32_t pad[1];
     /* dispatcher CTAs: landing areas for polls of the host ring (one is looked at while the next ones fly):
      * 32 descriptors as read from the ring, and a 33rd row for the control words that come with them */
     uint32_t stage[AESOFF_LANDINGS][33][AESOFF_STAGE_STRIDE];
@@ -591,18 +592,26 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
     unsigned long long token_at = (K == 1u) ? b_seq : 0ull; /* chain.next as last seen */
     bool queue_long = false;     /* the holder's last word on it */
     uint32_t empties = 0;        /* looks in a row that found nothing */
+    if (lane == 0) c->token_moved_us = (uint32_t)(globaltimer_ns() >> 10) - 1000u;
+    __syncwarp();
 
     for (;;) {
         /* ---- phase 1: the PCIe round trip ---------------------------------------------------- */
         {
             const bool holder = have_token || token_at == b_seq + pos;
-            const bool near = holder || (queue_long && token_at + 2ull * AESOFF_BATCH >= b_seq);
+            /* ... and the warp whose batch comes next reads its slots ahead once the holder has at most four requests
+             * of its batch left and the token has moved in the last few microseconds (traffic, not an idle engine whose
+             * token happens to rest there): without this, every 32nd request of a moderate stream waited for the next
+             * warp to wake up (3 us) and for its first poll (1.5 us) -- 1 MiB x 16: 729 -> 741 GB/s, p99 31.8 -> 29.1 us                    */
+            const uint32_t now_us = (uint32_t)(globaltimer_ns() >> 10);
+            const bool soon = !holder && b_seq + pos <= token_at + 4ull && now_us - lds_volatile(&c->token_moved_us) < 8u;
+            const bool near = holder || soon || (queue_long && token_at + 2ull * AESOFF_BATCH >= b_seq);
             /* The holder of the token, once it has found the ring empty (an idle engine: the latency case), keeps `depth` polls in flight, each issued when an older one has been looked at: a request
              * that arrives waits a fraction of a PCIe round trip for the next poll to leave instead of half of one
              * (lone 4 KiB 8.9 -> 8.25 us with three; 3 KiB per microsecond of PCIe reads).  Polls that were issued before
              * a request was taken would show it again: they are skipped, not looked at (see the end of the loop).   */
             const uint32_t depth = (holder && empties >= 1u) ? P.tune[AESOFF_TUNE_POLL_DEPTH] : 1u;
-            if (!holder && n_issued == n_looked) __nanosleep(queue_long ? 400u : 3000u); /* device words only: no PCIe read (ISSUE_POLL) */
+            if (!holder && !soon && n_issued == n_looked) __nanosleep(queue_long ? 400u : 3000u); /* device words only: no PCIe read (ISSUE_POLL) */
             while (n_issued - n_looked < depth) {
                 if (n_issued != n_looked) __nanosleep(P.tune[AESOFF_TUNE_POLL_GAP]); /* spread them over a round trip */
                 ISSUE_POLL(b_seq, pos, near);
@@ -641,6 +650,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         const unsigned long long idle = ((unsigned long long)a_idle.y << 32) | a_idle.x;
         const uint32_t quit_word = a_idle.z;
         queue_long = a_idle.w != 0u;
+        if (chain_next != token_at && lane == 0) sts_volatile(&c->token_moved_us, (uint32_t)(globaltimer_ns() >> 10));
         token_at = chain_next;
         wide = (n >= 8u) ? 1u : 0u;
         const uint32_t n_seen = n;
@@ -897,16 +907,6 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
 
         /* ---- phase 4: keys, descriptors, tickets ----------------------------------------------- */
         const uint32_t fine = UNIT_MODE(fine_max, half_min, 0u); /* of the request's first chunk (statistics, descriptor) */
-        {   /* statistics for aes_engine_info */
-            const uint32_t me = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_FINE));
-            const uint32_t mh = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_HALF));
-            if (lane == 0) { /* kept in shared memory, not in registers; written to the host when the ring is next found empty */
-                c->disp_stat[0] += __popc(me);
-                c->disp_stat[1] += __popc(mh);
-                c->disp_stat[2] += n - __popc(me) - __popc(mh);
-                c->disp_stat[3] = 1u;
-            }
-        }
         uint32_t keyloc = kw & 0xffffu;
         if (!(kw & AESOFF_KW_RAW) && keyloc >= AESOFF_KEY_IDS) keyloc = AESOFF_KEY_IDS + slot; /* never sent by the host */
         if (take && (kw & AESOFF_KW_RAW)) {
@@ -921,19 +921,6 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                 key_expand<6>(ybase, key, P.ktab[keyloc].rk);
             else
                 key_expand<8>(ybase, key, P.ktab[keyloc].rk);
-        }
-        if (take) {
-            /* the 24 descriptor words as 8 pieces of {3 words, tag}: see aesoff_dq_entry_t */
-            uint4 *d4 = reinterpret_cast<uint4 *>(P.dq + slot);
-            const uint32_t tg = (uint32_t)s;
-            d4[0] = p0; /* the first three pieces as they came (their tag is this request's) */
-            d4[1] = p1;
-            d4[2] = p2;
-            d4[3] = make_uint4(p3.x, kw >> 24, p3.z & 3u, tg);
-            d4[4] = make_uint4(nchunks, 1u << clog, (uint32_t)s, tg);
-            d4[5] = make_uint4((uint32_t)(s >> 32), rows, 0u, tg);
-            d4[6] = make_uint4((uint32_t)first_ticket, (uint32_t)(first_ticket >> 32), keyloc, tg);
-            d4[7] = make_uint4(0u, 0u, 0u, tg);
         }
 #undef PW
         /* expanded keys (if any request of this poll brought a raw one) before the tickets that point at
@@ -967,11 +954,37 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             }
         }
 #undef UNIT_MODE
+        /* the descriptors AFTER the tickets: a service warp that waits on a ticket reads it one L2 round trip after it
+         * is written and only then asks for the descriptor, whose pieces validate themselves (a piece read too early
+         * is read again); the eight stores per request used to stand between a request and its first ticket */
+        if (take) {
+            /* the 24 descriptor words as 8 pieces of {3 words, tag}: see aesoff_dq_entry_t */
+            uint4 *d4 = reinterpret_cast<uint4 *>(P.dq + slot);
+            const uint32_t tg = (uint32_t)s;
+            d4[0] = p0; /* the first three pieces as they came (their tag is this request's) */
+            d4[1] = p1;
+            d4[2] = p2;
+            d4[3] = make_uint4(p3.x, kw >> 24, p3.z & 3u, tg);
+            d4[4] = make_uint4(nchunks, 1u << clog, (uint32_t)s, tg);
+            d4[5] = make_uint4((uint32_t)(s >> 32), rows, 0u, tg);
+            d4[6] = make_uint4((uint32_t)first_ticket, (uint32_t)(first_ticket >> 32), keyloc, tg);
+            d4[7] = make_uint4(0u, 0u, 0u, tg);
+        }
         __syncwarp();
         /* What the service warps read, raised once the tickets are on their way.  Not a store: a dispatcher that got
          * the token later may already have published a larger count.  No fence: the count only tells the service warps
          * how many tickets they may reserve; a ticket is taken when its own 16-byte word shows up (tag).          */
         if (lane == 0 && total) atomicMax(g_published, new_pub);
+        {   /* statistics for aes_engine_info */
+            const uint32_t me = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_FINE));
+            const uint32_t mh = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_HALF));
+            if (lane == 0) { /* kept in shared memory, not in registers; written to the host when the ring is next found empty */
+                c->disp_stat[0] += __popc(me);
+                c->disp_stat[1] += __popc(mh);
+                c->disp_stat[2] += n - __popc(me) - __popc(mh);
+                c->disp_stat[3] = 1u;
+            }
+        }
         /* an empty request (len == 0) has no ticket: complete it here */
         if (take && nchunks == 0) {
             __threadfence_system();
