@@ -778,7 +778,8 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                                         (int)r0 <= fine_max, else half rows if (int)r0 >= half_min, else rows */
         /* (the dispatcher is one warp running dependent instructions, a few clocks each: a hundred instructions
          * on this path are 0.2 us on every request, so chunk sizes are powers of two and nothing here divides) */
-        uint32_t nchunks = 0, clog = P.chunk_log2; /* rows per chunk = 1 << clog */
+        uint32_t nchunks = 0, clog = P.chunk_log2; /* rows per chunk = 1 << clog ... */
+        uint32_t spread_rows = 0;                  /* ... unless this says otherwise (a lone request: one chunk per CTA) */
         {
             const unsigned long long bl = (pub_est > reserved ? pub_est - reserved : 0ull) << P.chunk_log2;
             const uint32_t backlog = bl > 0x3fffffffull ? 0x3fffffffu : (uint32_t)bl;
@@ -790,8 +791,10 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
                 rows <= gridDim.x * P.tune[AESOFF_TUNE_SPREAD_MAX]) { /* a lone request of moderate size */
                 /* longer requests keep chunk_rows: many tickets per CTA balance by themselves, and what a CTA may
                  * hold is counted in chunk_rows-sized tickets (service_loop) */
+                /* (not a power of two: 8 MiB is 2,048 rows, and 128 chunks of 16 would leave 20 of 148 CTAs without any;
+                 * the two divisions are paid by requests longer than one row per CTA only) */
                 clog = 0;
-                while ((gridDim.x << clog) < rows) ++clog;
+                if (rows > gridDim.x) spread_rows = (rows + gridDim.x - 1u) / gridDim.x;
             } else if (mine && may_cut && rows >= 4u * gridDim.x * AESOFF_WORKER_WARPS) {
                 /* a very long request (37 MiB and up): 16-row chunks, a quarter of the tickets -- cut into 4-row chunks a lone
                  * 64 MiB request ran at 747 GB/s, the service warps' ticket and descriptor traffic being what held it back;
@@ -804,7 +807,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             if (may_cut) {
                 if (idle_gpu)
                     fm = total_q <= P.tune[AESOFF_TUNE_FINE_TOTAL] ? 0x7fffffff
-                                                                   : (int)P.tune[AESOFF_TUNE_FINE_FRONT] - (int)ahead - (int)(1u << clog);
+                                                                   : (int)P.tune[AESOFF_TUNE_FINE_FRONT] - (int)ahead - (int)(spread_rows ? spread_rows : 1u << clog);
                 if (total_q <= P.tune[AESOFF_TUNE_HALF_TOTAL])
                     hm = 0;
                 else if (ahead <= P.tune[AESOFF_TUNE_TAIL_AHEAD])
@@ -818,7 +821,9 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             /* a request must fit the ticket ring with room to spare */
             while (((rows + (1u << clog) - 1u) >> clog) > P.TM / 4u) ++clog;
             nchunks = (rows + (1u << clog) - 1u) >> clog;
+            if (spread_rows) nchunks = (rows + spread_rows - 1u) / spread_rows;
         }
+        const uint32_t crows = spread_rows ? spread_rows : 1u << clog; /* rows per chunk of this lane's request */
         /* exclusive prefix sum of nchunks -> first ticket of each request */
         uint32_t incl = nchunks;
         if (n > 1) {
@@ -933,7 +938,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         if (take && nchunks <= 8u) {
             for (uint32_t ch = 0; ch < nchunks; ++ch) {
                 const unsigned long long tno = first_ticket + ch;
-                const uint32_t md = UNIT_MODE(fine_max, half_min, ch << clog) << AESOFF_TICKET_MODE_SHIFT;
+                const uint32_t md = UNIT_MODE(fine_max, half_min, ch * crows) << AESOFF_TICKET_MODE_SHIFT;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
                     make_uint4((uint32_t)s, ch | md, keyloc, (uint32_t)tno + 1u);
             }
@@ -943,12 +948,12 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             const uint32_t nc = __shfl_sync(0xffffffffu, nchunks, k);
             const unsigned long long ft = __shfl_sync(0xffffffffu, first_ticket, k);
             const uint32_t kl = __shfl_sync(0xffffffffu, keyloc, k);
-            const uint32_t cl = __shfl_sync(0xffffffffu, clog, k);
+            const uint32_t cl = __shfl_sync(0xffffffffu, crows, k);
             const uint32_t fm = __shfl_sync(0xffffffffu, fine_max, k), hm = __shfl_sync(0xffffffffu, half_min, k);
             const uint32_t sq = (uint32_t)(b_seq + k);
             for (uint32_t ch = lane; ch < nc; ch += 32) {
                 const unsigned long long tno = ft + ch;
-                const uint32_t md = UNIT_MODE(fm, hm, ch << cl) << AESOFF_TICKET_MODE_SHIFT;
+                const uint32_t md = UNIT_MODE(fm, hm, ch * cl) << AESOFF_TICKET_MODE_SHIFT;
                 *reinterpret_cast<uint4 *>(P.tmap + (tno & (unsigned long long)(P.TM - 1))) =
                     make_uint4(sq, ch | md, kl, (uint32_t)tno + 1u);
             }
@@ -965,7 +970,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
             d4[1] = p1;
             d4[2] = p2;
             d4[3] = make_uint4(p3.x, kw >> 24, p3.z & 3u, tg);
-            d4[4] = make_uint4(nchunks, 1u << clog, (uint32_t)s, tg);
+            d4[4] = make_uint4(nchunks, crows, (uint32_t)s, tg);
             d4[5] = make_uint4((uint32_t)(s >> 32), rows, 0u, tg);
             d4[6] = make_uint4((uint32_t)first_ticket, (uint32_t)(first_ticket >> 32), keyloc, tg);
             d4[7] = make_uint4(0u, 0u, 0u, tg);

@@ -95,6 +95,21 @@ def test_lengths_and_carries(P):
     _check(P, reqs)
 
 
+def test_lone_requests_one_chunk_per_cta(P):
+    """A lone request of more than one row per CTA is cut into ceil(rows / CTAs)-row chunks (not a power of
+    two: 3 MiB -> 6 rows, 5 MiB + 5 -> 9, 7 MiB - 16 -> 13, 9 MiB -> 16), a counter that carries out of bytes
+    14 and 13 inside it included.  One at a time, so that each finds the GPU idle; every byte checked."""
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7100]))
+    info = P.aes_engine_info()
+    icbs = [rng.bytes(8) + bytes(8), rng.bytes(12) + bytes([0x00, 0x00, 0xff, 0xf0]), rng.bytes(13) + bytes([0xff, 0xfe, 0x07])]
+    for j, n in enumerate(((3 << 20), (5 << 20) + 5, (7 << 20) - 16, 9 << 20, 577 * 4096 + 1)):
+        key = rng.bytes((16, 24, 32)[j % 3])
+        data = np.frombuffer(rng.bytes(n), dtype=np.uint8)
+        _check(P, [(key, icbs[j % 3], data)])
+    after = P.aes_engine_info()
+    assert after["running"] == 1 and after["kernel_launches"] == info["kernel_launches"]
+
+
 def test_config2_shape_64_in_flight(P):
     """configs[1] at reduced count: 64 x 1 MiB AES-128, one key, distinct nonces, all 64 in flight."""
     w = workloads.config2(n=64)
