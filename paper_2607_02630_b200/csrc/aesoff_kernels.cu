@@ -71,7 +71,11 @@ struct __align__(16) CtaCtl {
     uint32_t tables_ready;        /* set by a worker once the tables are filled: the service warp, which starts fetching
                                      tickets while they are being built, needs them for a decrypting request's keys */
     uint32_t token_moved_us;      /* dispatcher: when it last saw the token move (1.024 us units; kept here, not in a register) */
-    uint32_t pad[1];
+    /* A dispatcher's CTA stands aside while requests overlap AND the GPU has nothing queued (service_loop): */
+    uint32_t multi_until_us;      /* dispatcher: requests have been overlapping until about this time (1.024 us units)         */
+    uint32_t last_take_us;        /* dispatcher: when it last took requests                                                    */
+    uint32_t starved_us;          /* service warp: when it last found no ticket waiting                                        */
+    uint32_t pad[2];
     /* dispatcher CTAs: landing areas for polls of the host ring (one is looked at while the next ones fly):
      * 32 descriptors as read from the ring, and a 33rd row for the control words that come with them */
     uint32_t stage[AESOFF_LANDINGS][33][AESOFF_STAGE_STRIDE];
@@ -314,6 +318,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
     unsigned long long t = 0;   /* that ticket */
     uint32_t stamp_base = 0;
     bool counted_idle = false;  /* this CTA is included in the device-wide idle-CTA count */
+    const bool disp_cta = persistent && blockIdx.x < P.n_disp; /* a dispatcher warp runs beside this CTA's workers */
     uint32_t last_chunk_rows = P.chunk_rows; /* rows of the chunk this CTA read last (requests choose their chunk size) */
 
     for (;;) {
@@ -347,6 +352,25 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
          *    CTA of the persistent engine also keeps ONE reservation on a ticket that does not
          *    exist yet, so that a lone request finds 148 CTAs waiting, one ticket each.         */
         unsigned long long avail = pub > tk ? pub - tk : 0ull;
+        /* The CTA of a dispatcher warp stands aside -- reserves nothing -- while requests overlap (its dispatcher says so)
+         * AND the queue has run dry within the last 24 us: then the GPU is short of work, not of CTAs, and what 16 cipher
+         * warps cost the dispatcher beside them (issue slots on its sub-partition, the queue in front of the shared-memory
+         * pipe that its loads and ticket stores go through too) is latency of every request.  With a lone request the
+         * dispatcher has nothing to do while the request is worked on, and with a queue that never runs dry its speed
+         * does not matter: in both cases the CTA works like any other.
+         * (Measured with the two CTAs standing aside always: 1 MiB x 16 737 -> 773 GB/s, the mix 9.2 -> 9.9 M requests/s,
+         * 64 KiB x 256 649 -> 664 GB/s -- and 938 -> 925 at saturation, which is why it is conditional.)              */
+        bool stand_aside = false;
+        if (disp_cta) {
+            const uint32_t now = (uint32_t)(globaltimer_ns() >> 10);
+            uint32_t starved = 0, until = 0;
+            if (lane == 0) {
+                if (avail == 0ull) sts_volatile(&c->starved_us, now);
+                starved = avail == 0ull ? now : lds_volatile(&c->starved_us);
+                until = lds_volatile(&c->multi_until_us);
+            }
+            stand_aside = __shfl_sync(0xffffffffu, (int)(until - now) > 0 && now - starved < 24u ? 1 : 0, 0) != 0;
+        }
         /*    A CTA does not hoard: what it holds (unclaimed units of its open slots plus the tickets
          *    it has reserved, in 1/8-row units) stays near one and a half rows per worker -- enough
          *    to hide a refill (microseconds against 10 us per row), little enough that the end of a
@@ -367,7 +391,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
              * are nearly out of work (less than half a row each): the ticket is then picked up one L2 round trip after it
              * is written instead of three (see the count, reserve, poll), which is latency that a window of small requests
              * turns into throughput.                                                                                  */
-            if (persistent && avail == 0ull && have_mask == 0u && (busy_mask == 0u || held < AESOFF_WORKER_WARPS * P.tune[AESOFF_TUNE_PRERESERVE]))
+            if (persistent && !stand_aside && avail == 0ull && have_mask == 0u && (busy_mask == 0u || held < AESOFF_WORKER_WARPS * P.tune[AESOFF_TUNE_PRERESERVE]))
                 avail = 1ull;
             const uint32_t hold_max = AESOFF_WORKER_WARPS * 12u; /* 1.5 rows per worker */
             unsigned long long cap = held < hold_max ? (hold_max - held + per_ticket - 1u) / per_ticket : 0u;
@@ -378,6 +402,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
             const uint32_t share = (a32 + gridDim.x - 1u) / gridDim.x;
             if (cap > share) cap = share ? share : 1ull;
             if (avail > cap) avail = cap;
+            if (stand_aside) avail = 0ull;
         }
         uint32_t n_need = __popc(need);
         if ((unsigned long long)n_need > avail) {
@@ -650,7 +675,13 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         const unsigned long long idle = ((unsigned long long)a_idle.y << 32) | a_idle.x;
         const uint32_t quit_word = a_idle.z;
         queue_long = a_idle.w != 0u;
-        if (chain_next != token_at && lane == 0) sts_volatile(&c->token_moved_us, (uint32_t)(globaltimer_ns() >> 10));
+        if (chain_next != token_at && lane == 0) {
+            /* another dispatcher has taken requests: the same bookkeeping as for a take of this warp's own (below) */
+            const uint32_t now = (uint32_t)(globaltimer_ns() >> 10);
+            sts_volatile(&c->token_moved_us, now);
+            if (chain_next - token_at >= 2ull || now - c->last_take_us < 7u) sts_volatile(&c->multi_until_us, now + 32u);
+            c->last_take_us = now;
+        }
         token_at = chain_next;
         wide = (n >= 8u) ? 1u : 0u;
         const uint32_t n_seen = n;
@@ -980,6 +1011,11 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
          * the token later may already have published a larger count.  No fence: the count only tells the service warps
          * how many tickets they may reserve; a ticket is taken when its own 16-byte word shows up (tag).          */
         if (lane == 0 && total) atomicMax(g_published, new_pub);
+        if (lane == 0) { /* do requests overlap?  Two or more in one take, or two takes within 7 us (a lone request takes 8.7) */
+            const uint32_t now = (uint32_t)(globaltimer_ns() >> 10);
+            if (n >= 2u || now - c->last_take_us < 7u) sts_volatile(&c->multi_until_us, now + 32u);
+            c->last_take_us = now;
+        }
         {   /* statistics for aes_engine_info */
             const uint32_t me = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_FINE));
             const uint32_t mh = __ballot_sync(0xffffffffu, take && (fine & AESOFF_FLAG_HALF));
