@@ -318,11 +318,20 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
     unsigned long long t = 0;   /* that ticket */
     uint32_t stamp_base = 0;
     bool counted_idle = false;  /* this CTA is included in the device-wide idle-CTA count */
+    uint32_t my_mode = 0;       /* unit size of the chunk in this lane's slot */
     const bool disp_cta = persistent && blockIdx.x < P.n_disp; /* a dispatcher warp runs beside this CTA's workers */
     uint32_t last_chunk_rows = P.chunk_rows; /* rows of the chunk this CTA read last (requests choose their chunk size) */
 
     for (;;) {
-        const bool is_free = mine && lds_volatile(&c->busy[lane]) == 0u;
+        /* this lane's slot: busy word and claim word, read together and ahead of the two L2 reads below (the claim word is
+         * needed only after them, for what the CTA holds: read there, its shared-memory latency -- long while the workers
+         * keep the pipe full -- came on top of the L2 round trip in every iteration) */
+        uint32_t busy_w = 0, claim_w = 0;
+        if (mine) {
+            busy_w = lds_volatile(&c->busy[lane]);
+            claim_w = lds_volatile(&c->claim[lane]);
+        }
+        const bool is_free = mine && busy_w == 0u;
         const uint32_t busy_mask = __ballot_sync(0xffffffffu, mine && !is_free);
         const uint32_t have_mask = __ballot_sync(0xffffffffu, have);
         uint32_t need = __ballot_sync(0xffffffffu, is_free && !have);
@@ -379,9 +388,9 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
             const uint32_t per_ticket = last_chunk_rows * 8u; /* a reserved ticket that has not been read yet: as large as the last one */
             uint32_t held = 0;
             if (mine && !is_free) {
-                const uint32_t w = lds_volatile(&c->claim[lane]);
+                const uint32_t w = claim_w;
                 const uint32_t left = (w >> 16) > (w & 0xffffu) ? (w >> 16) - (w & 0xffffu) : 0u;
-                const uint32_t f = c->unit_mode[lane];
+                const uint32_t f = my_mode; /* this lane filled the slot: it knows the unit size (CtaCtl::unit_mode is for the workers) */
                 held = (f & AESOFF_FLAG_FINE) ? left : (f & AESOFF_FLAG_HALF) ? left * 4u : left * 8u * AESOFF_ROWS_PER_UNIT;
             } else if (have) {
                 held = per_ticket;
@@ -510,6 +519,7 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
                 sl->ring_slot = ring;
                 sl->n_units = n_units;
                 c->unit_mode[lane] = fine;
+                my_mode = fine;
                 sl->mode = sl->desc.flags & 3u;
                 c->done[lane] = 0u;
                 c->stamp[lane] = stamp_base + __popc(ready_mask & ((1u << lane) - 1u));
