@@ -60,6 +60,7 @@ extern "C" {
 #define AES_E_CUDA      -8   /* a CUDA runtime call failed / no device             */
 #define AES_E_BUSY      -9   /* call not allowed while the engine is running       */
 #define AES_E_NOMEM     -10  /* host or device allocation failed                   */
+#define AES_E_TOOBIG    -11  /* aes_ctr_launch_static: len > AES_STATIC_MAX_BYTES   */
 
 /* what a request computes (SP 800-38A sec. 6.5, 6.1, 6.2) */
 #define AES_MODE_CTR     0
@@ -264,6 +265,47 @@ int aes_mode_launch_batch(const int32_t *modes, aes_ctx_t *const *ctxs, const ui
                           const void *const *srcs, void *const *dsts,
                           const size_t *lens, size_t n,
                           int device, void *cuda_stream, uint32_t chunk_rows);
+
+/* ---- launch backend without allocation -----------------------------------------------------------
+ * aes_ctr_launch_batch obtains its device-side queue with cudaMalloc (and frees / re-obtains it when a batch
+ * outgrows it) and a staging buffer with cudaHostAlloc.  Some users of this library cannot do that:
+ *   - a server that handed all device memory to a pool of its own at start-up (a tensor framework's caching
+ *     allocator, a database's buffer pool): cudaMalloc fails there although the process owns the memory;
+ *   - a process with a kernel that never exits on that GPU (this library's persistent engine is one such
+ *     kernel; see aes_engine_start): cudaFree waits for it, i.e. for ever;
+ *   - a request handler that cannot afford the driver-wide lock and the tens of microseconds to milliseconds
+ *     a cudaMalloc / cudaFree costs in front of a 4 KiB offload.
+ * aes_ctr_launch_static is the launch backend for ONE CTR request (SP 800-38A sec. 6.5; the offload of
+ * PAPER.md:132, on the caller's stream as in PAPER.md:224) that allocates nothing, on the host or on the device:
+ * its queue -- counters, one descriptor, one expanded key, the tables, up to 1,024 chunk tickets -- lives in a
+ * 19.25 KiB array that is part of the library's image.  Every GPU on which the process loads the library holds
+ * that array until the process exits, used or not.  The request and its expanded key travel as the argument of a
+ * small set-up kernel; a second launch, the engine kernel in drain mode, does the work.  Both are enqueued on
+ * `cuda_stream` (a cudaStream_t of `device`, NULL = the legacy default stream); the call returns after
+ * enqueueing and the caller synchronises the stream or an event, as with aes_ctr_launch_batch.
+ *
+ *   ctx, nonce      host, as for aes_ctr_submit (nonce = the full 16-byte initial counter block).
+ *   src, dst        the caller's buffers, as for aes_ctr_submit: memory of `device`, or pinned host memory it can
+ *                   address; 16-byte aligned; dst == src allowed.  This call never owns or copies them.
+ *   len             0 .. AES_STATIC_MAX_BYTES (64 MiB).  More is refused with AES_E_TOOBIG and nothing is
+ *                   enqueued: the ticket array cannot grow.  Split a larger payload into pieces with the counter
+ *                   advanced by len / 16 per piece, or use aes_ctr_launch_batch.
+ *
+ * The first call on each device asks the CUDA runtime for the array's address on that GPU and copies the 2 KiB
+ * of tables into it with a synchronous cudaMemcpy; make that first call (len = 16 will do) while the process
+ * sets up, before any stream capture begins.  Later calls only launch.  The caller's current device is
+ * restored before returning.
+ *
+ * All calls on a device share the one array, and each call's set-up kernel rewrites the parts that the engine
+ * kernel expects to find zeroed or filled (ticket counter, countdown, descriptor, key, tickets) -- so two calls
+ * whose kernels can overlap on the GPU (different streams with no dependency between them) corrupt each other's
+ * queue.  Keep this entry point's calls on one stream per device, or order them with events.  Calls on the same
+ * stream may follow each other without any synchronisation in between.  The persistent engine must not be
+ * running on `device` (AES_E_BUSY: its CTAs hold the shared memory).
+ * Returns AES_OK, AES_E_INVAL, AES_E_ALIGN, AES_E_OVERLAP, AES_E_TOOBIG, AES_E_BUSY or AES_E_CUDA.             */
+#define AES_STATIC_MAX_BYTES (64u << 20)
+int aes_ctr_launch_static(aes_ctx_t *ctx, const uint8_t nonce[16], const void *src, void *dst, size_t len,
+                          int device, void *cuda_stream);
 
 /* ---- pinned host memory the GPU can address (for host-resident payloads) ----- */
 void *aes_host_alloc(size_t bytes);        /* NULL on error (AES_E_CUDA / AES_E_NOMEM) */

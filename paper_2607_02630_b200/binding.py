@@ -32,6 +32,8 @@ AES_E_STOPPED = -7
 AES_E_CUDA = -8
 AES_E_BUSY = -9
 AES_E_NOMEM = -10
+AES_E_TOOBIG = -11
+AES_STATIC_MAX_BYTES = 64 << 20
 
 
 class AesOffError(RuntimeError):
@@ -102,6 +104,7 @@ def _load() -> ctypes.CDLL:
         "aes_last_error": (i32, []),
         "aes_strerror": (ctypes.c_char_p, [i32]),
         "aes_ctr_launch_batch": (i32, [vp, vp, vp, vp, vp, sz, i32, vp, ctypes.c_uint32]),
+        "aes_ctr_launch_static": (i32, [vp, vp, vp, vp, sz, i32, vp]),
         "aes_host_alloc": (vp, [sz]),
         "aes_host_free": (None, [vp]),
         "aes_host_register": (i32, [vp, sz]),
@@ -121,7 +124,7 @@ def _load() -> ctypes.CDLL:
 _lib = _load()
 EXPORTS = ("aes_engine_start", "aes_engine_stop", "aes_engine_info", "aes_engine_info_device", "aes_engine_stop_device", "aes_route_flush", "aes_ctx_create", "aes_ctx_destroy",
            "aes_ctx_round_keys", "aes_ctr_submit", "aes_ecb_submit", "aes_cbc_decrypt_submit", "aes_mode_launch_batch", "aes_poll", "aes_wait", "aes_last_error", "aes_strerror",
-           "aes_ctr_launch_batch", "aes_host_alloc", "aes_host_free", "aes_host_register", "aes_host_unregister", "aes_loop_run", "aes_loop_run_mt", "aes_openloop_run", "aes_calibrate")
+           "aes_ctr_launch_batch", "aes_ctr_launch_static", "aes_host_alloc", "aes_host_free", "aes_host_register", "aes_host_unregister", "aes_loop_run", "aes_loop_run_mt", "aes_openloop_run", "aes_calibrate")
 
 
 def aes_strerror(code: int) -> str:
@@ -235,6 +238,14 @@ def aes_ctr_launch_batch(ctxs, nonces, srcs, dsts, lens, device: int = 0, cuda_s
     assert a_non.size == 16 * n and a_ctx.size == n and a_src.size == n and a_dst.size == n
     _check(_lib.aes_ctr_launch_batch(a_ctx.ctypes.data, a_non.ctypes.data, a_src.ctypes.data, a_dst.ctypes.data,
                                      a_len.ctypes.data, n, device, cuda_stream, chunk_rows), "aes_ctr_launch_batch")
+
+
+def aes_ctr_launch_static(ctx, nonce: bytes, src: int, dst: int, nbytes: int, device: int = 0, cuda_stream: int = 0) -> None:
+    """One CTR request through the launch backend that allocates nothing (its queue is a static device array of the
+    library, for callers that cannot cudaMalloc: see include/aesoff.h).  nbytes <= AES_STATIC_MAX_BYTES, else
+    AES_E_TOOBIG.  Enqueues on cuda_stream and returns; the caller synchronises."""
+    assert len(nonce) == 16
+    _check(_lib.aes_ctr_launch_static(ctx, bytes(nonce), src, dst, nbytes, device, cuda_stream), "aes_ctr_launch_static")
 
 
 AES_MODE_CTR, AES_MODE_ECB_ENC, AES_MODE_ECB_DEC, AES_MODE_CBC_DEC = 0, 1, 2, 3

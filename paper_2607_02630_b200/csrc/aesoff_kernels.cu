@@ -27,8 +27,13 @@
  */
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <string.h>
 
+#include <mutex>
+
+#include "aesoff.h"
 #include "aesoff_cipher.cuh"
+#include "aesoff_internal.h"
 #include "aesoff_shared.h"
 
 using namespace aesoff;
@@ -1132,4 +1137,218 @@ extern "C" int aesoff_launch_engine(const aesoff_params_t *params, int n_ctas, v
     const uint32_t smem = params->need_dec ? AESOFF_SMEM_BYTES : AESOFF_SMEM_BYTES_NODEC;
     aesoff_engine_kernel<<<n_ctas, AESOFF_CTA_THREADS, smem, (cudaStream_t)stream>>>(*params);
     return (int)cudaGetLastError();
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* aes_ctr_launch_static: the launch backend for callers that must not allocate                */
+/* ------------------------------------------------------------------------------------------ */
+/* Who this is for.  aes_ctr_launch_batch keeps its queue (counters, descriptors, keys, tickets) in
+ * device memory that it obtains with cudaMalloc on first use, frees and re-obtains when a batch
+ * outgrows it, and fills through a cudaHostAlloc'ed staging buffer.  Three kinds of user of this
+ * library cannot live with that:
+ *   - a server that gave the GPU's memory to an allocator of its own when it started (a tensor
+ *     framework's caching pool, a database's buffer pool): nothing is left, cudaMalloc answers
+ *     "out of memory" although the process holds plenty;
+ *   - a process in which some kernel never ends -- this library's own persistent engine on that
+ *     GPU is one (include/aesoff.h, aes_engine_start), other people's are others: cudaFree waits
+ *     for every kernel on the device, that one included, so the re-allocation above never returns;
+ *   - a request handler on a latency budget: cudaMalloc and cudaFree take driver-wide locks and
+ *     cost from tens of microseconds to milliseconds, more than the 4 KiB offload they would serve.
+ * For them the whole queue of ONE request lives in the array below.  It is part of the library's
+ * image: every GPU on which the process loads this library carries its AESOFF_STATIC_BYTES (19.25 KiB)
+ * from then until the process ends, whether or not this entry point is ever called.
+ *
+ * Inside host code `g_static_scratch` is not an address a kernel can use -- it names the host-side
+ * shadow of the symbol.  The address on a given GPU comes from cudaGetSymbolAddress, asked once per
+ * device with that device current (static_scratch_of); device code, like the set-up kernel, may name
+ * the array directly.
+ *
+ * Layout (offsets in bytes; every part starts on a multiple of 128):
+ *      0  counters          AESOFF_CNT_WORDS x 8    rewritten by every call's set-up kernel
+ *    512  dq_done           one countdown word       cleared by every call
+ *    640  dev_done_seq      one word
+ *    768  dq                ONE descriptor (the request), tagged pieces
+ *   1024  ktab              ONE expanded key
+ *   1280  T0 | Td0          2 KiB, written once per device by static_scratch_of and never again
+ *   3328  tmap              AESOFF_STATIC_TICKETS tickets of 16 bytes
+ */
+#define AESOFF_STATIC_TICKETS 1024u
+#define AESOFF_STATIC_OFF_DONE 512u
+#define AESOFF_STATIC_OFF_SEQ 640u
+#define AESOFF_STATIC_OFF_DQ 768u
+#define AESOFF_STATIC_OFF_KEY 1024u
+#define AESOFF_STATIC_OFF_T0 1280u
+#define AESOFF_STATIC_OFF_TMAP 3328u
+#define AESOFF_STATIC_BYTES (AESOFF_STATIC_OFF_TMAP + AESOFF_STATIC_TICKETS * 16u)
+
+static __device__ __align__(256) uint8_t g_static_scratch[AESOFF_STATIC_BYTES];
+
+extern "C" int aesoff_fail(int code);          /* aesoff_runtime.cpp: files the code for aes_last_error() */
+extern "C" void aesoff_note_launches(int n);   /* aesoff_runtime.cpp: aes_engine_info_t::kernel_launches   */
+
+namespace {
+
+/* everything the set-up kernel needs, passed by value as its kernel argument (376 bytes) */
+struct StaticJob {
+    aesoff_dev_desc_t desc; /* the request as the service warps read it */
+    uint32_t rk[60];        /* its expanded key                          */
+    uint32_t total;         /* tickets = chunks of the request           */
+    uint32_t crows;         /* rows per chunk                            */
+    uint64_t rows;
+    uint64_t wave;          /* rows the grid's worker warps take at once */
+};
+
+/* Writes the call's queue into the static array.  The array still holds the previous call's queue, so every
+ * word the engine kernel reads before writing is stored here again: all counters (the ticket counter must
+ * start at 0), the chunk countdown, the completion word, the descriptor, the key and tickets 0 .. total-1.
+ * Tickets past `total` are stale but never reserved (drain_total).                                        */
+__global__ void __launch_bounds__(256) aesoff_static_setup_kernel(const StaticJob J)
+{
+    uint8_t *base = g_static_scratch; /* device code names the array itself */
+    const uint32_t tid = threadIdx.x;
+    unsigned long long *cnt = reinterpret_cast<unsigned long long *>(base);
+    if (tid < AESOFF_CNT_WORDS) cnt[tid] = (tid == AESOFF_CNT_PUBLISHED) ? (unsigned long long)J.total : 0ull;
+    if (tid == 64) *reinterpret_cast<uint32_t *>(base + AESOFF_STATIC_OFF_DONE) = 0u;
+    if (tid == 65) *reinterpret_cast<unsigned long long *>(base + AESOFF_STATIC_OFF_SEQ) = 0ull;
+    if (tid >= 96 && tid < 128) { /* descriptor word p at w[(p / 3) * 4 + p % 3], tag = sequence number 1 */
+        const uint32_t i = tid - 96u, q = i >> 2, r = i & 3u;
+        const uint32_t *w = reinterpret_cast<const uint32_t *>(&J.desc);
+        reinterpret_cast<uint32_t *>(base + AESOFF_STATIC_OFF_DQ)[i] = (r == 3u) ? 1u : w[3u * q + r];
+    }
+    if (tid >= 128 && tid < 192) {
+        const uint32_t i = tid - 128u;
+        reinterpret_cast<uint32_t *>(base + AESOFF_STATIC_OFF_KEY)[i] = i < 60u ? J.rk[i] : 0u;
+    }
+    /* the same end-of-launch rule as aes_ctr_launch_batch: the chunks that hold the last wave of rows are cut
+     * into 1/8 rows, the four waves before them into half rows                                              */
+    for (uint32_t c = tid; c < J.total; c += blockDim.x) {
+        const unsigned long long left = J.rows - (unsigned long long)c * J.crows;
+        const uint32_t mode = left <= J.wave ? AESOFF_FLAG_FINE : left <= 5ull * J.wave ? AESOFF_FLAG_HALF : 0u;
+        reinterpret_cast<uint4 *>(base + AESOFF_STATIC_OFF_TMAP)[c] =
+            make_uint4(1u, c | (mode << AESOFF_TICKET_MODE_SHIFT), 0u, c + 1u);
+    }
+}
+
+std::mutex g_static_mu;
+uint8_t *g_static_ptr[AESOFF_MAX_DEVICES]; /* device address of g_static_scratch on each GPU, once known */
+int g_static_sms[AESOFF_MAX_DEVICES];
+
+/* Set-up, once per device, with that device current: asks the runtime where the array lives on THIS GPU and
+ * puts the two tables there.  The copy is a synchronous cudaMemcpy: this is why the first call on a device
+ * belongs before any stream capture.  Returns NULL on error.                                              */
+uint8_t *static_scratch_of(int device)
+{
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    if (g_static_ptr[device]) return g_static_ptr[device];
+    int sms = 0, major = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device) != cudaSuccess || major != 10 || sms <= 0)
+        return nullptr;
+    uint8_t *ptr = nullptr;
+    if (cudaGetSymbolAddress((void **)&ptr, g_static_scratch) != cudaSuccess || !ptr) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    if (cudaMemcpy(ptr + AESOFF_STATIC_OFF_T0, aesoff_T0_table(), 512 * 4, cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        return nullptr;
+    }
+    g_static_sms[device] = sms;
+    g_static_ptr[device] = ptr;
+    return ptr;
+}
+
+} /* namespace */
+
+extern "C" __attribute__((visibility("default"))) int aes_ctr_launch_static(aes_ctx_t *ctx, const uint8_t nonce[16],
+                                                                            const void *src, void *dst, size_t len,
+                                                                            int device, void *cuda_stream)
+{
+    if (!ctx || !nonce) return aesoff_fail(AES_E_INVAL);
+    if (len > (size_t)AES_STATIC_MAX_BYTES) return aesoff_fail(AES_E_TOOBIG);
+    if (len == 0) return AES_OK;
+    if (!src || !dst) return aesoff_fail(AES_E_INVAL);
+    const uintptr_t s = (uintptr_t)src, d = (uintptr_t)dst;
+    if ((s | d) & 15u) return aesoff_fail(AES_E_ALIGN);
+    if (s != d && s < d + len && d < s + len) return aesoff_fail(AES_E_OVERLAP);
+    if (device < 0 || device >= AESOFF_MAX_DEVICES) return aesoff_fail(AES_E_INVAL);
+    aes_engine_info_t info;
+    if (aes_engine_info_device(device, &info) == AES_OK && info.running) return aesoff_fail(AES_E_BUSY);
+
+    StaticJob J;
+    memset(&J, 0, sizeof(J));
+    uint8_t rkb[240];
+    const int nr = aes_ctx_round_keys(ctx, rkb); /* host expansion, done once per context */
+    if (nr < 0) return nr;
+    memcpy(J.rk, rkb, (size_t)16 * (nr + 1));    /* little-endian host: FIPS byte string == little-endian-loaded words */
+
+    /* geometry: rows of 256 counter values aligned on counter byte 15 == 0; chunks of 4 rows, doubled until
+     * the request fits the ticket array (64 MiB: 16,385 rows -> 513 chunks of 32)                          */
+    const uint64_t nblocks = ((uint64_t)len + 15u) >> 4;
+    const uint64_t rows = (nblocks + nonce[15] + AESOFF_ROW_BLOCKS - 1) >> 8;
+    uint32_t crows = 4;
+    while ((rows + crows - 1) / crows > AESOFF_STATIC_TICKETS) crows *= 2;
+    const uint32_t total = (uint32_t)((rows + crows - 1) / crows);
+
+    int ndev = 0, prev = -1;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev || cudaGetDevice(&prev) != cudaSuccess) {
+        cudaGetLastError();
+        return aesoff_fail(AES_E_CUDA);
+    }
+    if (prev != device && cudaSetDevice(device) != cudaSuccess) {
+        cudaGetLastError();
+        return aesoff_fail(AES_E_CUDA);
+    }
+    int rc = AES_OK;
+    uint8_t *ptr = static_scratch_of(device);
+    if (!ptr) {
+        rc = AES_E_CUDA;
+    } else {
+        memcpy(J.desc.icb, nonce, 16);
+        J.desc.src = (uint64_t)s;
+        J.desc.dst = (uint64_t)d;
+        J.desc.len = (uint64_t)len;
+        J.desc.nr = (uint32_t)nr;
+        J.desc.flags = AESOFF_MODE_CTR;
+        J.desc.nchunks = total;
+        J.desc.chunk_rows = crows;
+        J.desc.seq = 1;
+        J.desc.rows = rows;
+        J.desc.first_ticket = 0;
+        J.desc.keyloc = 0;
+        J.total = total;
+        J.crows = crows;
+        J.rows = rows;
+        J.wave = (uint64_t)g_static_sms[device] * AESOFF_WORKER_WARPS;
+
+        aesoff_params_t p;
+        memset(&p, 0, sizeof(p));
+        p.counters = reinterpret_cast<uint64_t *>(ptr);
+        p.dq_done = reinterpret_cast<uint32_t *>(ptr + AESOFF_STATIC_OFF_DONE);
+        p.dev_done_seq = reinterpret_cast<uint64_t *>(ptr + AESOFF_STATIC_OFF_SEQ);
+        p.dq = reinterpret_cast<aesoff_dq_entry_t *>(ptr + AESOFF_STATIC_OFF_DQ);
+        p.ktab = reinterpret_cast<aesoff_key_t *>(ptr + AESOFF_STATIC_OFF_KEY);
+        p.T0 = reinterpret_cast<const uint32_t *>(ptr + AESOFF_STATIC_OFF_T0);
+        p.tmap = reinterpret_cast<aesoff_ticket_t *>(ptr + AESOFF_STATIC_OFF_TMAP);
+        p.drain_total = total;
+        p.R = 1;                       /* one request: every sequence number maps to entry 0 */
+        p.TM = AESOFF_STATIC_TICKETS;
+        p.chunk_rows = crows;
+        p.mode = AESOFF_MODE_DRAIN;
+        p.first_seq = 1;
+        uint64_t ctas = (rows + AESOFF_ROWS_PER_CTA - 1) / AESOFF_ROWS_PER_CTA;
+        if (ctas > (uint64_t)g_static_sms[device]) ctas = (uint64_t)g_static_sms[device];
+        cudaStream_t stream = (cudaStream_t)cuda_stream;
+        aesoff_static_setup_kernel<<<1, 256, 0, stream>>>(J);
+        if (cudaGetLastError() != cudaSuccess || aesoff_launch_engine(&p, (int)ctas, stream) != 0) {
+            cudaGetLastError();
+            rc = AES_E_CUDA;
+        } else {
+            aesoff_note_launches(2);
+        }
+    }
+    explicit_bzero(&J, sizeof(J)); /* key hygiene: the expanded key was on this stack frame */
+    explicit_bzero(rkb, sizeof(rkb));
+    if (prev != device) cudaSetDevice(prev);
+    return rc == AES_OK ? AES_OK : aesoff_fail(rc);
 }

@@ -253,6 +253,10 @@ int check_buffers(const void *src, void *dst, size_t len)
 /* ============================================================================================ */
 extern "C" int aes_last_error(void) { return t_last_error; }
 
+/* for aes_ctr_launch_static, which lives beside its static array in aesoff_kernels.cu */
+extern "C" int aesoff_fail(int code) { return fail(code); }
+extern "C" void aesoff_note_launches(int n) { g_kernel_launches.fetch_add((uint64_t)n); }
+
 extern "C" const char *aes_strerror(int code)
 {
     switch (code) {
@@ -267,6 +271,7 @@ extern "C" const char *aes_strerror(int code)
     case AES_E_CUDA: return "CUDA error or no device";
     case AES_E_BUSY: return "not allowed while the engine is running";
     case AES_E_NOMEM: return "out of memory";
+    case AES_E_TOOBIG: return "request larger than AES_STATIC_MAX_BYTES (aes_ctr_launch_static has no memory to grow into)";
     default: return "unknown error";
     }
 }
