@@ -160,9 +160,12 @@ int aes_engine_info_device(int device, aes_engine_info_t *out);
  * Requests are independent ("each offload belongs to one request"), so the path
  * shards over the GPUs of a node with NO exchange step: aes_engine_start() may be called once per device
  * (up to 8 per process), and aes_ctr_submit() sends each request to the engine of the GPU that owns its
- * dst, else its src (cudaPointerGetAttributes, remembered per 2 MiB page and per thread); requests whose
- * src and dst are both host memory go round the running engines.  A request whose memory belongs to a GPU
- * without a running engine fails with AES_E_STOPPED.  With one engine running nothing is looked up.  A
+ * device buffer(s) (cudaPointerGetAttributes on src and dst, remembered per 2 MiB page and per thread);
+ * requests whose src and dst are both host memory go round the running engines.  A request whose memory
+ * belongs to a GPU without a running engine fails with AES_E_STOPPED -- also when only one engine runs on a
+ * node with several GPUs.  A request whose src belongs to one GPU and whose dst to another fails with
+ * AES_E_INVAL: the engine's kernel would have to dereference a peer pointer, and this library never enables
+ * peer access.  Only on a node with ONE GPU is nothing looked up.  A
  * handle carries its engine in its top byte; aes_poll / aes_wait take handles of any engine.  A context
  * may be used on all engines (its key is filed per engine).  NVLink is not used, no collective runs.
  * aes_engine_stop() stops every running engine, aes_engine_stop_device() one.  aes_route_flush() forgets
@@ -195,7 +198,7 @@ int aes_ctx_round_keys(const aes_ctx_t *ctx, uint8_t *out);
  * T_{j+1} = (T_j + 1) mod 2^128 read as a big-endian integer; a final partial
  * block uses the leading len mod 16 bytes of its O_n.  No padding.
  *
- *   ctx    host; round keys are copied into the descriptor before this returns.
+ *   ctx    host; the key (raw, or the index of its installed expansion) is copied into the descriptor before this returns.
  *   nonce  host; the FULL 16-byte initial counter block T_1 (BASELINE.json
  *          configs[0]: 8-byte nonce || 8-byte big-endian counter from 0); copied.
  *   src    DEVICE pointer on the engine's GPU, or pinned host memory that the GPU
@@ -207,7 +210,8 @@ int aes_ctx_round_keys(const aes_ctx_t *ctx, uint8_t *out);
  *   len    any value >= 0 and < 2^36 (64 GiB); len == 0 completes without touching memory.
  *
  * Never blocks.  Returns the handle (>= 1), or 0 with aes_last_error() in
- * {AES_E_INVAL, AES_E_ALIGN, AES_E_OVERLAP, AES_E_AGAIN (ring full), AES_E_STOPPED}.
+ * {AES_E_INVAL (also: src and dst on two different GPUs), AES_E_ALIGN, AES_E_OVERLAP, AES_E_AGAIN (ring full),
+ * AES_E_STOPPED (also: the GPU that owns the memory runs no engine)}.
  * Requests may complete out of order.                                            */
 aes_handle_t aes_ctr_submit(aes_ctx_t *ctx, const uint8_t nonce[16],
                             const void *src, void *dst, size_t len);

@@ -146,8 +146,8 @@ __global__ void __launch_bounds__(CALIB_THREADS, 2) calib_copy_kernel(const uint
  * cipher's own main-round instruction mix.  Returns 0 or a CUDA error.                                   */
 extern "C" int aesoff_run_calibration(int device, double out[8])
 {
-    cudaError_t e = cudaSetDevice(device);
-    if (e != cudaSuccess) return (int)e;
+    AesoffDeviceScope on_device(device); /* the caller's current device is restored on return */
+    if (!on_device.ok) return (int)cudaErrorInvalidDevice;
     int sms = 0;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     const uint32_t iters = 4096;

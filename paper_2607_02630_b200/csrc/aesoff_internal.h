@@ -41,10 +41,31 @@ struct aes_ctx {
 /* Which engine a request goes to (aesoff_router.cpp; "requests routed to the GPU that owns
  * their src/dst").  owner: device index of the memory, AESOFF_OWNER_HOST for host memory.                        */
 #define AESOFF_OWNER_HOST (-2)
+#define AESOFF_ROUTE_NONE  (-1) /* aesoff_route_decide: nothing runs, or the owner of the memory runs no engine */
+#define AESOFF_ROUTE_MIXED (-2) /* src and dst belong to two different GPUs */
 int aesoff_route_decide(int src_owner, int dst_owner, uint32_t running_mask, uint32_t *round_robin);
 typedef int (*aesoff_owner_fn)(const void *ptr); /* resolves the owner of an address (cudaPointerGetAttributes) */
 int aesoff_route_owner_cached(const void *ptr, aesoff_owner_fn resolve);
 void aesoff_route_flush_cache(void);
+
+/* Makes `device` current for a scope and puts the caller's device back at its end: a process that runs torch (or an
+ * engine) on another GPU must not find its later allocations moved because it called into this library.        */
+#ifdef __CUDA_RUNTIME_H__
+struct AesoffDeviceScope {
+    int prev = -1, target = -1;
+    bool ok = false;
+    explicit AesoffDeviceScope(int device) : target(device)
+    {
+        ok = cudaGetDevice(&prev) == cudaSuccess && (prev == device || cudaSetDevice(device) == cudaSuccess);
+    }
+    ~AesoffDeviceScope()
+    {
+        if (ok && prev != target) cudaSetDevice(prev);
+    }
+    AesoffDeviceScope(const AesoffDeviceScope &) = delete;
+    AesoffDeviceScope &operator=(const AesoffDeviceScope &) = delete;
+};
+#endif
 
 const uint32_t *aesoff_T0_table();
 int aesoff_key_expand(const uint8_t *key, int keybits, uint32_t rk[60]);

@@ -4,11 +4,13 @@
  * PAPER.md:25, 105-107) and so are the blocks inside one: the path shards with NO exchange step, so the
  * router is a table look-up, not a collective:
  *
- *   - device memory decides: a request runs on the GPU that owns dst (the bytes it writes), else on the one
- *     that owns src; moving a payload over NVLink to encrypt it elsewhere would cost about what the cipher does;
+ *   - device memory decides: a request runs on the GPU that owns its device buffer(s); moving a payload over
+ *     NVLink to encrypt it elsewhere would cost about what the cipher does;
+ *   - src on one GPU and dst on another is refused (AESOFF_ROUTE_MIXED): an engine's kernel dereferences both,
+ *     and this library never enables peer access, so whichever engine took it would fault and lose all it holds;
  *   - a request whose src and dst are both host memory (the paper's j.buf) may run anywhere:
  *     the running engines take such requests in turn;
- *   - with ONE engine running everything goes there and no address is looked at (the one-GPU fast path).
+ *   - with ONE engine running on a node with ONE GPU everything goes there and no address is looked at.
  *
  * Owners are resolved by the caller's function (cudaPointerGetAttributes in the runtime, a table in the CPU
  * tests) and remembered per 2 MiB page in a small per-thread cache: allocations of different devices never
@@ -23,7 +25,8 @@
 
 int aesoff_route_decide(int src_owner, int dst_owner, uint32_t running_mask, uint32_t *round_robin)
 {
-    if (running_mask == 0) return -1;
+    if (running_mask == 0) return AESOFF_ROUTE_NONE;
+    if (src_owner >= 0 && dst_owner >= 0 && src_owner != dst_owner) return AESOFF_ROUTE_MIXED;
     if (dst_owner >= 0) return ((running_mask >> dst_owner) & 1u) ? dst_owner : -1; /* its owner has no engine: refuse */
     if (src_owner >= 0) return ((running_mask >> src_owner) & 1u) ? src_owner : -1;
     /* host memory on both sides: the running engines in turn */
@@ -94,7 +97,7 @@ extern "C" __attribute__((visibility("default"))) uint64_t aesoff_test_route_man
     uint32_t rr = 0;
     for (size_t i = 0; i < n; ++i) {
         const int dO = aesoff_route_owner_cached((const void *)(uintptr_t)dsts[i], synthetic_owner);
-        const int so = dO < 0 ? aesoff_route_owner_cached((const void *)(uintptr_t)srcs[i], synthetic_owner) : AESOFF_OWNER_HOST;
+        const int so = aesoff_route_owner_cached((const void *)(uintptr_t)srcs[i], synthetic_owner);
         out[i] = aesoff_route_decide(so, dO, running_mask, &rr);
     }
     return t_resolver_calls;

@@ -144,21 +144,34 @@ int resolve_owner(const void *ptr)
     return a.type == cudaMemoryTypeDevice ? a.device : AESOFF_OWNER_HOST;
 }
 
-/* the engine a request goes to, or nullptr (none running / the owner of its memory runs none) */
-Engine *route(const void *src, void *dst, size_t len)
+/* GPUs of the node (cudaGetDeviceCount at the last engine start) and the test hook AESOFF_ROUTE_ALWAYS=1, read at every
+ * engine start: owners are looked up even where the answer cannot matter (one GPU, one engine), so that the look-up path
+ * can be exercised against real CUDA addresses on a one-GPU box (tests/test_gpu_router.py).                            */
+std::atomic<int> g_node_gpus{0};
+std::atomic<int> g_route_always{0};
+
+/* The engine a request goes to, or nullptr with *err = AES_E_STOPPED (none running / the GPU that owns its memory runs
+ * none) or AES_E_INVAL (src and dst belong to two different GPUs: no engine can reach both -- peer access is never
+ * enabled, include/aesoff.h).  Owners are not looked at only where there is nothing to decide and nothing to refuse: one
+ * engine on a node with one GPU.  With one engine on a node with several GPUs the look-up stays (one remembered answer per
+ * 2 MiB page and thread): memory of another GPU must be refused, not handed to a kernel that cannot address it.          */
+Engine *route(const void *src, void *dst, size_t len, int *err)
 {
+    *err = AES_E_STOPPED;
     const int single = g_single.load(std::memory_order_acquire);
-    if (single >= 0) return &g_engs[single];
+    if (single >= 0 && g_node_gpus.load(std::memory_order_relaxed) == 1 && !g_route_always.load(std::memory_order_relaxed))
+        return &g_engs[single];
     const uint32_t mask = g_running_mask.load(std::memory_order_acquire);
     if (mask == 0) return nullptr;
     int so = AESOFF_OWNER_HOST, dO = AESOFF_OWNER_HOST;
     if (len) {
         dO = aesoff_route_owner_cached(dst, resolve_owner);
-        if (dO < 0) so = aesoff_route_owner_cached(src, resolve_owner);
+        so = src == dst ? dO : aesoff_route_owner_cached(src, resolve_owner);
     }
     uint32_t rr = g_round_robin.load(std::memory_order_relaxed);
     const int d = aesoff_route_decide(so, dO, mask, &rr);
     if (so < 0 && dO < 0) g_round_robin.store(rr, std::memory_order_relaxed);
+    if (d == AESOFF_ROUTE_MIXED) *err = AES_E_INVAL;
     return d >= 0 ? &g_engs[d] : nullptr;
 }
 std::atomic<uint64_t> g_kernel_launches{0};
@@ -388,7 +401,13 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(AES_E_CUDA);
-    if (cudaSetDevice(device) != cudaSuccess) return fail(AES_E_CUDA);
+    g_node_gpus.store(ndev, std::memory_order_relaxed);
+    {
+        const char *ra = getenv("AESOFF_ROUTE_ALWAYS");
+        g_route_always.store(ra && ra[0] == '1', std::memory_order_relaxed);
+    }
+    AesoffDeviceScope on_device(device); /* the caller's current device is restored on every return below */
+    if (!on_device.ok) return fail(AES_E_CUDA);
     int sms = 0, major = 0;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
@@ -504,7 +523,12 @@ extern "C" int aes_engine_start(int device, const aes_engine_opts_t *opts)
     const uint64_t t0 = now_ns();
     while (__atomic_load_n(&e.hctl[AESOFF_CTL_ALIVE], __ATOMIC_ACQUIRE) == 0u) {
         if (now_ns() - t0 > 20ull * 1000000000ull || cudaStreamQuery(e.stream) != cudaErrorNotReady) {
+            /* A kernel that was only waiting for the SMs may still start: it must find STOP in memory that is still
+             * mapped, so the stream is waited for (the kernel sees STOP and leaves, or has failed) before anything
+             * is freed.                                                                                            */
             __atomic_store_n(&e.hctl[AESOFF_CTL_STOP], 1u, __ATOMIC_RELEASE);
+            cudaStreamSynchronize(e.stream);
+            cudaGetLastError();
             free_engine_memory(e);
             return fail(AES_E_CUDA);
         }
@@ -680,9 +704,10 @@ aes_handle_t submit_mode(aes_ctx_t *ctx, uint32_t mode, const uint8_t nonce[16],
         fail(rc);
         return 0;
     }
-    Engine *ep = route(src, dst, len);
+    int route_err = AES_E_STOPPED;
+    Engine *ep = route(src, dst, len, &route_err);
     if (!ep) {
-        fail(AES_E_STOPPED);
+        fail(route_err);
         return 0;
     }
     Engine &e = *ep;
@@ -974,7 +999,8 @@ extern "C" int aes_mode_launch_batch(const int32_t *modes, aes_ctx_t *const *ctx
     }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) return fail(AES_E_CUDA);
-    if (cudaSetDevice(device) != cudaSuccess) return fail(AES_E_CUDA);
+    AesoffDeviceScope on_device(device); /* the caller's current device is restored on every return below */
+    if (!on_device.ok) return fail(AES_E_CUDA);
     int sms = 0, major = 0;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
     cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);

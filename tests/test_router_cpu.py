@@ -21,9 +21,10 @@ def decide(src, dst, mask, rr):
     return L.aesoff_test_route_decide(src, dst, mask, ctypes.byref(rr))
 
 
-def test_device_memory_decides_dst_first():
+def test_device_memory_decides_and_two_owners_are_refused():
     rr = ctypes.c_uint32(0)
-    assert decide(3, 5, 0xFF, rr) == 5          # dst wins
+    assert decide(3, 5, 0xFF, rr) == -2         # src on GPU 3, dst on GPU 5: no engine reaches both (AES_E_INVAL)
+    assert decide(5, 5, 0xFF, rr) == 5
     assert decide(3, HOST, 0xFF, rr) == 3       # host dst: src decides
     assert decide(HOST, 6, 0xFF, rr) == 6
     assert rr.value == 0                        # no round-robin turn was spent on them
@@ -58,7 +59,7 @@ def test_routes_over_a_synthetic_address_map_and_the_page_cache():
     page = rng.integers(0, 4, size=n)
     off = rng.integers(0, 1 << 17, size=n) * 16
     dsts = np.asarray([_dev_addr(int(d), int(p) * (1 << 21) + int(o)) for d, p, o in zip(dev, page, off)], dtype=np.uint64)
-    srcs = dsts + np.uint64(1 << 20)
+    srcs = np.asarray([_dev_addr(int(d), int(p) * (1 << 21)) for d, p in zip(dev, page)], dtype=np.uint64)  # same page, same owner
     out = np.zeros(n, dtype=np.int32)
     calls = L.aesoff_test_route_many(srcs.ctypes.data, dsts.ctypes.data, n, 0xFF, out.ctypes.data, 1)
     assert (out == dev).all()
@@ -85,6 +86,10 @@ def test_host_buffers_mixed_with_device_buffers():
     assert out[3] == 6 and out[5] == 2
     rest = [int(out[i]) for i in range(8) if i not in (3, 5)]
     assert rest == [0, 2, 6, 0, 2, 6]
+    # src on GPU 0, dst on GPU 2, both with an engine: refused (-2 -> AES_E_INVAL), whichever is looked at first
+    srcs[1], dsts[1] = _dev_addr(0, 256), _dev_addr(2, 512)
+    L.aesoff_test_route_many(srcs.ctypes.data, dsts.ctypes.data, 8, 0b01000101, out.ctypes.data, 1)
+    assert out[1] == -2 and out[3] == 6 and out[5] == 2
 
 
 def test_handles_name_their_engine_and_bad_ones_are_invalid():
