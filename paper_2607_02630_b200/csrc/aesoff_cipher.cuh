@@ -15,8 +15,10 @@
  *     builds the whole lookup address  (byte_k(x) << 8) | lane*4 | region_base.
  *   - CTR structure: a warp works on one "row" = the 256 counter values that share the upper 120
  *     counter bits.  Everything of rounds 1 and 2 that depends only on those bits is computed once
- *     per row; per block round 1 is ONE lookup and round 2 FOUR (133 instead of 160 lookups per
- *     AES-128 block, 197 instead of 224 for AES-256).
+ *     per row; per block round 1 is ONE lookup and round 2 FOUR: 133 lookups per AES-128 block in
+ *     the row's step instead of 160, 197 instead of 224 for AES-256 -- 135.3 / 199.3 once the row
+ *     set-up (27 + 10 lookups per lane for a pair of rows = 16 blocks) is counted in, the figure
+ *     bench.py's roofline uses.
  *   - Payload is read/written with 128-bit L2-only accesses (ld.global.cg / st.global.cg): a
  *     persistent kernel never gets its L1 invalidated, so a recycled request buffer must not hit L1.
  */

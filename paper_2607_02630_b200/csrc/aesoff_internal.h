@@ -12,11 +12,13 @@
  *   second submit       as above, and that dispatcher also stores the expanded key at ktab[id]
  *   until that request has COMPLETED (mailbox)   raw key again, nothing stored: several dispatcher warps
  *                       take requests side by side, so "submitted earlier" does not mean "expanded earlier"
- *   afterwards          the descriptor only names ktab[id]                                       */
+ *   afterwards          the descriptor only names ktab[id]
+ * An id belongs to one generation of the key table (epoch): INSTALLED or INSTALLING under an older epoch starts over. */
 #define AESOFF_CTX_FRESH      0u
 #define AESOFF_CTX_SEEN       1u
 #define AESOFF_CTX_INSTALLING 2u
 #define AESOFF_CTX_INSTALLED  3u
+#define AESOFF_CTX_CLAIMED    4u /* transient: one thread is writing id / epoch / install_seq on its way to INSTALLING */
 
 #define AESOFF_MAX_DEVICES 8 /* engines per process: one per GPU of a node */
 

@@ -18,9 +18,10 @@
  *                 the device-wide ticket counter, polls them until the dispatcher has written them,
  *                 copies the 96-byte descriptor and the 240-byte expanded key into the slot and opens
  *                 it for claiming -- all while the workers are busy with earlier slots.
- *   warp 17       DISPATCHER (CTA 0, persistent mode only).  Polls the host-mapped descriptor ring
- *                 over PCIe (one round trip per batch of up to 32 requests), expands keys that arrive
- *                 raw (step a1), and cuts each request into chunk tickets (step a3).
+ *   warp 17       DISPATCHER (CTAs 0 .. n_dispatchers-1, persistent mode only).  Polls the host-mapped
+ *                 descriptor ring over PCIe (one round trip per batch of up to 32 requests; batches go
+ *                 round the dispatcher warps), expands keys that arrive raw (step a1), and cuts each
+ *                 request into chunk tickets (step a3).
  * Completion (step a7): the worker that finishes the last unit of a slot counts the request's chunks
  * down in global memory; the last chunk's finisher fences at system scope and writes the request's
  * sequence number into the host-mapped mailbox.
@@ -324,7 +325,9 @@ __device__ void service_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t ybase
     uint32_t stamp_base = 0;
     bool counted_idle = false;  /* this CTA is included in the device-wide idle-CTA count */
     uint32_t my_mode = 0;       /* unit size of the chunk in this lane's slot */
-    const bool disp_cta = persistent && blockIdx.x < P.n_disp; /* a dispatcher warp runs beside this CTA's workers */
+    /* a dispatcher warp runs beside this CTA's workers.  Such a CTA may stand aside (below) only while CTAs without a
+     * dispatcher remain to take the tickets: in a grid of at most n_disp CTAs (n_ctas = 1 or 2 is allowed) nobody stands aside */
+    const bool disp_cta = persistent && blockIdx.x < P.n_disp && gridDim.x > P.n_disp;
     uint32_t last_chunk_rows = P.chunk_rows; /* rows of the chunk this CTA read last (requests choose their chunk size) */
 
     for (;;) {
@@ -777,7 +780,7 @@ __device__ void dispatcher_loop(const aesoff_params_t &P, CtaCtl *c, uint32_t yb
         }
 
         /* ---- phase 2: what does not depend on the token: the rows of request pos + k ---------------- */
-        /* (32-bit row counts: the host refuses requests of 2^40 bytes and more) */
+        /* (32-bit row counts: the host refuses requests of 2^36 bytes and more, check_buffers) */
         const bool mine = lane >= pos && lane < pos + n;
         uint32_t rows = 0;
 #define PW(p) sw[AESOFF_PW_INDEX(p)]

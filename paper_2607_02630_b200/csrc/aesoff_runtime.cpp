@@ -266,6 +266,13 @@ int check_buffers(const void *src, void *dst, size_t len)
 /* ============================================================================================ */
 extern "C" int aes_last_error(void) { return t_last_error; }
 
+/* test hook (tests/test_gpu_restart.py): where a context's key stands on one engine, AESOFF_CTX_* */
+extern "C" __attribute__((visibility("default"))) int aesoff_test_ctx_state(const aes_ctx_t *ctx, int device)
+{
+    if (!ctx || device < 0 || device >= AESOFF_MAX_DEVICES) return -1;
+    return (int)__atomic_load_n(&ctx->dev[device].state, __ATOMIC_ACQUIRE);
+}
+
 /* for aes_ctr_launch_static, which lives beside its static array in aesoff_kernels.cu */
 extern "C" int aesoff_fail(int code) { return fail(code); }
 extern "C" void aesoff_note_launches(int n) { g_kernel_launches.fetch_add((uint64_t)n); }
@@ -732,9 +739,17 @@ aes_handle_t submit_mode(aes_ctx_t *ctx, uint32_t mode, const uint8_t nonce[16],
      * batches of requests side by side, so a lower sequence number alone does not mean "expanded first". */
     uint32_t kw = ((uint32_t)ctx->nr << 24) | AESOFF_KEY_NONE | AESOFF_KW_RAW;
     bool installing = false;
-    uint32_t st = __atomic_load_n(&ck.state, __ATOMIC_ACQUIRE);
-    const uint64_t epoch_now = e.k_epoch.load(std::memory_order_acquire);
-    const bool epoch_ok = __atomic_load_n(&ck.epoch, __ATOMIC_ACQUIRE) == epoch_now;
+    /* state and epoch are two words: read the state again after the epoch and start over if another thread moved it in
+     * between (a re-install after a rebuilt key table goes INSTALLED/INSTALLING -> CLAIMED -> INSTALLING with the NEW epoch;
+     * a stale INSTALLED paired with the new epoch would name a table entry that has not been filled yet)               */
+    uint32_t st;
+    uint64_t epoch_now;
+    bool epoch_ok;
+    do {
+        st = __atomic_load_n(&ck.state, __ATOMIC_ACQUIRE);
+        epoch_now = e.k_epoch.load(std::memory_order_acquire);
+        epoch_ok = __atomic_load_n(&ck.epoch, __ATOMIC_ACQUIRE) == epoch_now;
+    } while (__atomic_load_n(&ck.state, __ATOMIC_ACQUIRE) != st);
     if (st == AESOFF_CTX_INSTALLING && epoch_ok) {
         const uint64_t is = __atomic_load_n(&ck.install_seq, __ATOMIC_ACQUIRE);
         if (is != 0 && __atomic_load_n(&e.hmail[(is - 1) & e.Rm], __ATOMIC_ACQUIRE) >= is) {
@@ -746,15 +761,18 @@ aes_handle_t submit_mode(aes_ctx_t *ctx, uint32_t mode, const uint8_t nonce[16],
         kw = ((uint32_t)ctx->nr << 24) | ck.id;
     } else if (st == AESOFF_CTX_FRESH) {
         __atomic_compare_exchange_n(&ck.state, &st, AESOFF_CTX_SEEN, false, __ATOMIC_ACQ_REL, __ATOMIC_ACQUIRE);
-    } else if (st == AESOFF_CTX_SEEN || (st == AESOFF_CTX_INSTALLED && !epoch_ok)) {
-        /* INSTALLED under an older ktab generation (the engine was rebuilt): install again */
+    } else if (st == AESOFF_CTX_SEEN || ((st == AESOFF_CTX_INSTALLED || st == AESOFF_CTX_INSTALLING) && !epoch_ok)) {
+        /* INSTALLED, or INSTALLING with nobody having looked at the install's completion yet, under an older ktab
+         * generation (the engine was rebuilt, or stopped uncleanly): install again.  The winner holds the entry in
+         * CLAIMED while it fills id, epoch and install_seq, so INSTALLING always comes with a consistent triple.    */
         const uint32_t id = alloc_key_id(e);
         if (id != AESOFF_KEY_NONE) {
-            if (__atomic_compare_exchange_n(&ck.state, &st, AESOFF_CTX_INSTALLING, false, __ATOMIC_ACQ_REL,
+            if (__atomic_compare_exchange_n(&ck.state, &st, AESOFF_CTX_CLAIMED, false, __ATOMIC_ACQ_REL,
                                             __ATOMIC_ACQUIRE)) {
                 __atomic_store_n(&ck.install_seq, 0ull, __ATOMIC_RELEASE);
                 ck.id = id;
                 __atomic_store_n(&ck.epoch, epoch_now, __ATOMIC_RELEASE);
+                __atomic_store_n(&ck.state, AESOFF_CTX_INSTALLING, __ATOMIC_RELEASE);
                 kw |= AESOFF_KW_INSTALL;
                 kw = (kw & ~0xffffu) | id;
                 installing = true;
@@ -763,7 +781,7 @@ aes_handle_t submit_mode(aes_ctx_t *ctx, uint32_t mode, const uint8_t nonce[16],
                 e.id_free.emplace_front(id, 0ull);
             }
         }
-    } /* else: INSTALLING and not complete yet (or another thread is in the middle of it): raw, nothing stored */
+    } /* else: INSTALLING and not complete yet, or CLAIMED (another thread is in the middle of it): raw, nothing stored */
     /* claim the next sequence number, but only if its slot has been vacated */
     uint64_t s = e.next_seq.load(std::memory_order_acquire);
     for (;;) {

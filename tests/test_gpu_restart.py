@@ -34,6 +34,50 @@ def test_installed_context_survives_restart():
     B.aes_ctx_destroy(ctx)
 
 
+def test_half_installed_context_starts_over_after_a_rebuilt_key_table():
+    """A context used exactly twice has asked for its key to be filed (INSTALLING) and nobody has looked at that
+    request's completion yet.  When the key table is rebuilt in that state (another ring size), the next submit must
+    file the key again and the one after it must find it INSTALLED -- not ship the raw key with every request for ever."""
+    import ctypes
+
+    import gpu_util as G
+    import paper_2607_02630_b200.binding as B
+    from oracle import oracle as o
+
+    state = B._lib.aesoff_test_ctx_state
+    state.restype, state.argtypes = ctypes.c_int, [ctypes.c_void_p, ctypes.c_int]
+    INSTALLING, INSTALLED = 2, 3
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE, 7705]))
+    key = rng.bytes(24)
+    data = np.frombuffer(rng.bytes(9000), dtype=np.uint8)
+    src, dst = G.to_device(data), G.device_empty(len(data))
+    G.stream_sync()
+    ctx = B.aes_ctx_create(key)
+
+    def once():
+        icb = rng.bytes(16)
+        B.aes_wait(B.aes_ctr_submit(ctx, icb, src.data_ptr(), dst.data_ptr(), len(data)))
+        assert dst.cpu().numpy().tobytes() == o.ctr(key, icb, data)
+
+    B.aes_engine_start(0, ring_slots=512, idle_exit_ms=60000)
+    try:
+        once()
+        once()
+        assert state(ctx, 0) == INSTALLING
+    finally:
+        B.aes_engine_stop()
+    B.aes_engine_start(0, ring_slots=128, idle_exit_ms=60000)  # other geometry: the key table is rebuilt
+    try:
+        once()
+        assert state(ctx, 0) == INSTALLING  # filed again, under the new table
+        once()
+        assert state(ctx, 0) == INSTALLED
+        once()
+    finally:
+        B.aes_engine_stop()
+    B.aes_ctx_destroy(ctx)
+
+
 def test_idle_exit_is_detected_and_engine_restarts():
     """Failure detection: a persistent kernel that has exited -- here by its own idle
     timer -- is seen through the host-mapped alive word: submits fail with AES_E_STOPPED instead of hanging,
