@@ -123,9 +123,13 @@ __device__ __forceinline__ void fill_td(uint32_t tbase, const uint32_t *Td0, uin
 template <int K>
 __device__ __forceinline__ uint32_t td(uint32_t x, uint32_t ybd)
 {
-    const uint32_t sh = (K == 0) ? (x << 7) : (x >> (8 * K - 7));
-    uint32_t v;
-    asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"((sh & 0x7f80u) | ybd));
+    /* The inverse rounds are bound by the ALU pipe (ncu, profiles/r3_ncu_modes.md: 97.7 % busy with shift + mask-or per
+     * address), so the address costs that pipe ONE instruction -- PRMT pulls the byte out -- and the scaling by the
+     * 128-byte entry stride plus the base goes to the FMA pipe as an integer multiply-add, which otherwise idles.     */
+    const uint32_t b = __byte_perm(x, 0u, 0x4440u | K);
+    uint32_t a, v;
+    asm("mad.lo.u32 %0, %1, 128, %2;" : "=r"(a) : "r"(b), "r"(ybd));
+    asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a));
     return v;
 }
 __device__ __forceinline__ uint32_t xor_bytes(uint32_t t) /* InvSubBytes(x) from Td0[x] */
