@@ -287,6 +287,11 @@ def main():
     ap.add_argument("--sweep-out", default="", help="with --sweep / --openloop: also write the table to this JSON file")
     ap.add_argument("--openloop", action="store_true", help="latency under Poisson load, blocking vs overlapping (PAPER.md:244)")
     ap.add_argument("--openloop-bytes", type=int, default=4096)
+    ap.add_argument("--dispatchers", type=int, default=0, help="with --dispatch-stats: dispatcher warps of the engine (0 = the default)")
+    ap.add_argument("--dispatch-stats", action="store_true",
+                    help="tuning aid, needs a library built with AESOFF_NVCC_EXTRA=-DAESOFF_DISP_STATS: what the dispatcher warps did "
+                         "(requests per take, time from a poll landing to the token, time from the token to the last ticket) "
+                         "while fine-grained cells ran under load")
     ap.add_argument("--plumbing-check", action="store_true",
                     help="run only the N-rank bookkeeping (rank discovery, host barrier, max-over-ranks reduction) on gloo, "
                          "no GPU work: what the CPU tests drive with two ranks")
@@ -299,6 +304,8 @@ def main():
         return run_openloop(args)
     if args.table2:
         return run_table2(args)
+    if args.dispatch_stats:
+        return run_dispatch_stats(args)
     if args.warmup < 3:
         args.warmup = 3
     if args.mode != "ctr":
@@ -859,6 +866,80 @@ def run_table2(args):
     if args.sweep_out:
         with open(args.sweep_out, "w") as f:
             json.dump({"rows": rows}, f, indent=1)
+    return 0
+
+
+def run_dispatch_stats(args):
+    """Where the dispatch pipeline's time goes under load (a request at 256 in flight takes twice as long as a
+    lone one).  Per cell, on a fresh engine of a -DAESOFF_DISP_STATS build: the closed loop's rate and latency, and per
+    dispatcher warp its polls that took requests ("takes"), requests per take, the time from a poll landing to the token
+    arriving (parse, geometry and waiting for the dispatcher before it) and from the token to the last ticket store (key
+    expansion, descriptor and ticket stores, fences), by the GPU's globaltimer."""
+    import ctypes
+
+    import torch
+
+    import paper_2607_02630_b200.binding as B
+
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    torch.zeros(1, device=dev)
+    torch.cuda.synchronize()
+    get = B._lib.aesoff_debug_dispatch_stats
+    get.restype, get.argtypes = ctypes.c_int, [ctypes.c_void_p]
+    rng = np.random.Generator(np.random.Philox(key=[workloads.SEED_BASE + 9, 1]))
+    pool = torch.empty(256 * MIB, dtype=torch.uint8, device=dev)
+    ctx = B.aes_ctx_create(rng.bytes(16))
+
+    def read_stats(ndisp):
+        time.sleep(0.05)  # the counters reach the host-mapped words at the first empty poll after the run
+        raw = (ctypes.c_uint32 * 40)()
+        assert get(raw) == 0
+        out = []
+        for d in range(ndisp):
+            takes, reqs, wait, work, empty = [int(raw[5 * d + i]) for i in range(5)]
+            if takes == 0:
+                continue
+            out.append({"dispatcher": d, "takes": takes, "requests_per_take": reqs / takes, "wait_us_per_take": wait * 0.064 / takes,
+                        "work_us_per_take": work * 0.064 / takes, "work_us_per_request": work * 0.064 / max(reqs, 1), "empty_polls": empty})
+        return out
+
+    cells = {}
+
+    def fixed(name, size, depth, nreq, threads=1):
+        B.aes_engine_start(0, idle_exit_ms=30000, n_dispatchers=args.dispatchers)
+        nd = B.aes_engine_info()["n_dispatchers"]
+        nbuf = max(depth, 64)
+        ptrs = np.asarray([pool.data_ptr() + (i % nbuf) * size for i in range(nreq)], dtype=np.uint64)
+        icb = rng.integers(0, 256, size=(nreq, 16), dtype=np.uint8)
+        lens = np.full(nreq, size, dtype=np.uint64)
+        c = run_cell(B, ptrs, icb, lens, depth, ctx, threads=threads, reps=3)
+        c["in_flight"], c["executor_threads"] = depth, threads
+        c["dispatchers"] = read_stats(nd)
+        B.aes_engine_stop()
+        cells[name] = c
+
+    fixed("aes128_4KiB_w1", 4096, 1, 20000)
+    fixed("aes128_4KiB_w256", 4096, 256, 150000)
+    fixed("aes128_4KiB_w256_threads4", 4096, 256, 150000, threads=4)
+    fixed("aes128_4KiB_w1024_threads4", 4096, 1024, 150000, threads=4)
+    fixed("aes128_64KiB_w256", 65536, 256, 150000)
+    for th in (1, 4):
+        B.aes_engine_start(0, idle_exit_ms=30000, n_dispatchers=args.dispatchers)
+        nd = B.aes_engine_info()["n_dispatchers"]
+        m = mix_c4(B, torch, dev, threads=(th,))
+        m["dispatchers"] = read_stats(nd)
+        B.aes_engine_stop()
+        cells["mix_c4_threads%d" % th] = m
+    B.aes_ctx_destroy(ctx)
+    if not any(c["dispatchers"] for c in cells.values()):
+        raise SystemExit("bench.py --dispatch-stats: all counters are zero: build the library with "
+                         "AESOFF_NVCC_EXTRA=-DAESOFF_DISP_STATS python -m paper_2607_02630_b200.build --force")
+    out = {"dispatch_stats": cells, "how": run_dispatch_stats.__doc__.split("\n\n")[0].replace("\n    ", " ")}
+    print(json.dumps(out))
+    if args.sweep_out:
+        with open(args.sweep_out, "w") as f:
+            json.dump(out, f, indent=1)
     return 0
 
 
